@@ -1,0 +1,216 @@
+"""ctypes front end of the CPU FP64 oracle (oracle/numa_oracle.c).
+
+TEST INFRASTRUCTURE.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+``--impl reference`` leg may import this.  It imports nothing from the product package
+``paper_2504_08157_b200`` and shares no code with the CUDA path.
+
+`Oracle` strings the C functions together in the order of SURVEY.md 8(a) / DESIGN.md:
+A0 setup -> (A2-A6 tendency + weight) -> A7 DSS -> A8 sources -> A9 walls -> A10 RK stage,
+A11 = SSP-RK3 (Shu-Osher) driver (reading Q11).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "numa_oracle.c")
+_LIB = os.path.join(_HERE, "libnuma_oracle.so")
+
+# SSP-RK3 (Shu-Osher) as (a0, a1, b):  q_out = a0 q0 + a1 qs + b dt L(qs)
+SSP_RK3 = ((1.0, 0.0, 1.0), (0.75, 0.25, 0.25), (1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0))
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain -O2, OpenMP over elements, no FP contraction)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-std=c99", "-shared", "-fPIC",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def _p(a, typ=C.c_double):
+    if a is None:
+        return None
+    return a.ctypes.data_as(C.POINTER(typ))
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_lgl.argtypes = [C.c_int, _dp, _dp]
+        L.orc_dmat.argtypes = [C.c_int, _dp, _dp]
+        L.orc_metrics.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp]
+        L.orc_metrics.restype = C.c_long
+        L.orc_mass.argtypes = [C.c_int, C.c_long, C.c_long, C.POINTER(C.c_int32), _dp, _dp, _dp, _dp]
+        L.orc_wall_list.argtypes = [C.c_int, C.c_long, C.POINTER(C.c_uint8), _dp,
+                                    C.POINTER(C.c_int64), _dp]
+        L.orc_wall_list.restype = C.c_long
+        L.orc_tendency.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.orc_weight.argtypes = [C.c_long, C.c_int, _dp, _dp, _dp]
+        L.orc_dss.argtypes = [C.c_long, C.c_long, C.c_int, C.POINTER(C.c_int32), _dp]
+        L.orc_sources.argtypes = [C.c_long, _dp, _dp, _dp, C.c_double, _dp]
+        L.orc_walls.argtypes = [C.c_long, C.c_long, C.POINTER(C.c_int64), _dp, _dp]
+        L.orc_rk_stage.argtypes = [C.c_long, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
+        _lib = L
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def lgl(N):
+    xi = np.empty(N + 1); w = np.empty(N + 1)
+    lib().orc_lgl(N, _p(xi), _p(w))
+    return xi, w
+
+
+def dmat(N):
+    xi, _ = lgl(N)
+    D = np.empty((N + 1, N + 1))
+    lib().orc_dmat(N, _p(xi), _p(D))
+    return D
+
+
+def metrics(N, xyz):
+    xyz = _f64(xyz)
+    Ne = xyz.shape[1]
+    met = np.empty((9,) + xyz.shape[1:])
+    jac = np.empty(xyz.shape[1:])
+    bad = lib().orc_metrics(N, Ne, _p(xyz), _p(met), _p(jac))
+    return met, jac, int(bad)
+
+
+def mass(N, intma_cg, n_global, jac):
+    intma_cg = np.ascontiguousarray(intma_cg, dtype=np.int32)
+    Ne = intma_cg.shape[0]
+    wJ = np.empty(jac.shape); M = np.empty(n_global); om = np.empty(jac.shape)
+    lib().orc_mass(N, Ne, n_global, _p(intma_cg, C.c_int32), _p(_f64(jac)), _p(wJ), _p(M), _p(om))
+    return wJ, M, om
+
+
+def wall_list(N, face_bc, met):
+    face_bc = np.ascontiguousarray(face_bc, dtype=np.uint8)
+    Ne = face_bc.shape[0]
+    cnt = lib().orc_wall_list(N, Ne, _p(face_bc, C.c_uint8), _p(met), None, None)
+    node = np.empty(cnt, dtype=np.int64); nrm = np.empty((cnt, 3))
+    if cnt:
+        lib().orc_wall_list(N, Ne, _p(face_bc, C.c_uint8), _p(met), _p(node, C.c_int64), _p(nrm))
+    return node, nrm
+
+
+def tendency(N, par, q, ref, met, want_T=False):
+    q = _f64(q); ref = _f64(ref)
+    Ne = q.shape[1]
+    S = np.empty_like(q)
+    T = np.empty_like(q) if want_T else None
+    par = _f64(par)
+    lib().orc_tendency(N, Ne, _p(par), _p(q), _p(ref), _p(met), _p(S), _p(T))
+    return (S, T) if want_T else S
+
+
+def weight(omega, S):
+    r = np.empty_like(S)
+    lib().orc_weight(omega.size, S.shape[0], _p(omega), _p(_f64(S)), _p(r))
+    return r
+
+
+def dss(intma_cg, n_global, r):
+    """In place on r[nf][Ne][Mn]."""
+    assert r.flags.c_contiguous and r.dtype == np.float64
+    intma_cg = np.ascontiguousarray(intma_cg, dtype=np.int32)
+    lib().orc_dss(intma_cg.size, n_global, r.shape[0], _p(intma_cg, C.c_int32), _p(r))
+    return r
+
+
+def sources(q, heat, beta, f_cor, r):
+    assert r.flags.c_contiguous
+    NL = q[0].size
+    lib().orc_sources(NL, _p(_f64(q)), _p(None if heat is None else _f64(heat)),
+                      _p(None if beta is None else _f64(beta)), float(f_cor), _p(r))
+    return r
+
+
+def walls(node, nrm, r):
+    assert r.flags.c_contiguous
+    NL = r[0].size
+    lib().orc_walls(NL, node.size, _p(node, C.c_int64), _p(nrm), _p(r))
+    return r
+
+
+def rk_stage(a0, a1, b_dt, q0, qs, r, out=None):
+    if out is None:
+        out = np.empty_like(q0)
+    lib().orc_rk_stage(q0.size, a0, a1, b_dt, _p(q0), _p(qs), _p(r), _p(out))
+    return out
+
+
+class Oracle:
+    """A0 once, then rhs()/step_rk3() on element-local SoA arrays [m][Ne][Mn]."""
+
+    def __init__(self, N, xyz, intma_cg, n_global, face_bc, ref, constants, f_cor=0.0,
+                 sponge=None):
+        self.N = N
+        self.intma_cg = np.ascontiguousarray(intma_cg, dtype=np.int32)
+        self.n_global = int(n_global)
+        self.ref = _f64(ref)
+        self.par = np.array([constants["g"], constants["p_a"], constants["R_gas"],
+                             constants["c_p"], constants["c_v"]], dtype=np.float64)
+        self.f_cor = float(f_cor)
+        self.sponge = None if sponge is None else _f64(sponge)
+        self.met, self.jac, bad = metrics(N, xyz)
+        if bad:
+            raise ValueError("non-positive Jacobian at %d nodes" % bad)
+        self.wJ, self.M, self.omega = mass(N, self.intma_cg, self.n_global, self.jac)
+        self.wall_node, self.wall_normal = wall_list(N, face_bc, self.met)
+
+    @classmethod
+    def from_workload(cls, wl):
+        m = wl.mesh
+        return cls(m.N, m.xyz, m.intma_cg, m.n_global, m.face_bc, wl.ref, wl.constants,
+                   f_cor=wl.f_cor, sponge=wl.sponge)
+
+    # --- the separate calls of the C-ABI boundary -------------------------------------
+    def rhs_local(self, q, want_T=False):
+        """numa_rhs: A2-A6, weighted element-local contributions (before DSS)."""
+        out = tendency(self.N, self.par, q, self.ref, self.met, want_T)
+        if want_T:
+            S, T = out
+            return weight(self.omega, S), weight(self.omega, T)
+        return weight(self.omega, out)
+
+    def dss(self, r):
+        """numa_dss_or_flux (CG): A7, in place."""
+        return dss(self.intma_cg, self.n_global, r)
+
+    def apply_sources(self, q, heat, r):
+        """numa_apply_sources: A8 then A9, in place."""
+        sources(q, heat, self.sponge, self.f_cor, r)
+        walls(self.wall_node, self.wall_normal, r)
+        return r
+
+    def rhs(self, q, heat=None):
+        """Full assembled tendency L(q) = walls(sources(DSS(omega * S(q))))."""
+        r = self.rhs_local(q)
+        self.dss(r)
+        self.apply_sources(q, heat, r)
+        return r
+
+    def step_rk3(self, q, dt, heat=None):
+        """A11: one SSP-RK3 step (Q11)."""
+        q0 = _f64(q)
+        qs = q0
+        for (a0, a1, b) in SSP_RK3:
+            r = self.rhs(qs, heat)
+            qs = rk_stage(a0, a1, b * dt, q0, qs, r)
+        return qs

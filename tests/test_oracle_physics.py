@@ -1,0 +1,279 @@
+"""Pins P7, P8, P9, P11, P13, P16 of the CPU oracle: the tendency of
+PAPER.md Eq. 1-3 against closed forms, conservation, a manufactured solution whose exact
+S(q) is derived symbolically from Eq. 1 and Eq. 3 as printed, and a NumPy Kronecker /
+sparse-matrix brute-force restatement on tiny meshes.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2504_08157_b200 import inputs
+
+C = inputs.CONSTANTS
+
+
+def _oracle(wl):
+    return orc.Oracle.from_workload(wl)
+
+
+# ---------------------------------------------------------------------------------------
+def test_P7_atmosphere_at_rest_is_bitwise_at_rest():
+    """u = 0, rho' = theta' = 0  =>  p' = expm1(0) = 0, F = 0  =>  L(q) == 0 exactly, on
+    deformed and stretched meshes, both backgrounds, and stays so over RK3 steps."""
+    for cfg, scale in ((1, 1.0), (3, 0.04)):
+        wl = inputs.make_workload(cfg, scale=scale)
+        o = _oracle(wl)
+        q = np.zeros_like(wl.q)
+        r = o.rhs(q, wl.heating * 0.0 if wl.heating is not None else None)
+        assert np.all(r == 0.0)
+        for _ in range(3):
+            q = o.step_rk3(q, wl.dt)
+        assert np.all(q == 0.0)
+
+
+def test_P8_buoyancy_closed_form():
+    """Config 1 at t = 0 (pressure-balanced bubble, u = 0): r_w = -(rho'/rho) g node by node
+    (Eq. 1b's last term); r_rho and r_theta are exactly 0 (products with u = 0);
+    r_u, r_v contain only round-off of grad p'.  Also shows DSS.omega leaves continuous
+    pointwise terms unchanged."""
+    wl = inputs.make_workload(1)
+    o = _oracle(wl)
+    r = o.rhs(wl.q)
+    rho = wl.ref[0] + wl.q[0]
+    expect = -(wl.q[0] / rho) * C["g"]
+    assert np.max(np.abs(expect)) > 0.015  # 0.5 K / 300 K * g
+    assert np.max(np.abs(r[3] - expect)) < 1e-9 * np.max(np.abs(expect))
+    assert np.all(r[0] == 0.0) and np.all(r[4] == 0.0)
+    assert np.max(np.abs(r[1])) < 1e-10 and np.max(np.abs(r[2])) < 1e-10
+
+
+@pytest.mark.parametrize("N", [2, 3, 4, 7])
+def test_P9_global_mass_conservation(N):
+    """sum_I M_I r_rho,I = sum_e sum wJ div F_N = closed-surface integral of F_N.n = 0 for
+    trilinear elements, planar walls with u.n = 0, N >= 2 (integrand degree <= 2N-1 per
+    direction, nodal flux single-valued across interior faces)."""
+    mesh = inputs.box_mesh(N, 3, 3, 2, (300.0, 300.0, 200.0), perturb=0.05, seed=21)
+    rho0, theta0 = inputs.reference_neutral(mesh.xyz[2])
+    q = inputs.smooth_random_state(mesh, rho0, theta0, seed=5)
+    # polynomial-in-reference-space fields are needed for the exactness argument: the nodal
+    # interpolant of any field IS such a polynomial, and F = rho*u is formed nodally.
+    o = orc.Oracle(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc,
+                   np.stack((rho0, theta0)), C)
+    r = o.rhs(q)
+    total = np.sum(o.wJ * r[0])
+    scale = np.sum(o.wJ * np.abs(r[0]))
+    assert scale > 0
+    assert abs(total) < 2e-13 * scale
+
+
+def test_P9_mass_conservation_fails_for_N1():
+    mesh = inputs.box_mesh(1, 3, 3, 2, (300.0, 300.0, 200.0), perturb=0.1, seed=21)
+    rho0, theta0 = inputs.reference_neutral(mesh.xyz[2])
+    q = inputs.smooth_random_state(mesh, rho0, theta0, seed=5)
+    o = orc.Oracle(1, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc,
+                   np.stack((rho0, theta0)), C)
+    r = o.rhs(q)
+    assert abs(np.sum(o.wJ * r[0])) > 1e-8 * np.sum(o.wJ * np.abs(r[0]))
+
+
+def test_P9_mass_drift_over_100_steps_config1():
+    wl = inputs.make_workload(1)
+    o = _oracle(wl)
+    q = wl.q
+    m0 = np.sum(o.wJ * q[0])
+    mref = np.sum(o.wJ * wl.ref[0])
+    for _ in range(100):
+        q = o.step_rk3(q, wl.dt)
+    assert np.all(np.isfinite(q))
+    assert abs(np.sum(o.wJ * q[0]) - m0) < 1e-13 * mref
+    assert np.max(np.abs(q[3])) > 1e-2  # the bubble did start to rise
+
+
+# ---------------------------------------------------------------------------------------
+def _manufactured(L):
+    """Smooth periodic fields on [0,L]^3 and the exact S(q) of Eq. 1 with Eq. 3 exactly as
+    printed (p = p_a (rho R theta / p_a)^gamma, p' = p - p0), g = 0, uniform background,
+    derived symbolically -- an independent route to the tendency."""
+    import sympy as sp
+    x, y, z = sp.symbols("x y z")
+    k = 2 * sp.pi / L
+    rho0, theta0 = sp.Rational(6, 5), 300
+    rhop = rho0 * sp.Rational(1, 50) * sp.sin(k * x) * sp.cos(k * y) * sp.cos(2 * k * z)
+    u = 5 * sp.sin(k * x + sp.Rational(1, 3)) * sp.cos(k * z)
+    v = -3 * sp.cos(k * y) * sp.sin(2 * k * x) + 1
+    w = 2 * sp.sin(k * z) * sp.cos(k * y + sp.Rational(1, 5))
+    thp = 2 * sp.cos(k * x) * sp.sin(k * y) * sp.cos(k * z) + sp.Rational(1, 2) * sp.sin(2 * k * z)
+    p_a, R, cp, cv = (sp.Float(C[n], 30) for n in ("p_a", "R_gas", "c_p", "c_v"))
+    gamma = cp / cv
+    rho = rho0 + rhop
+    theta = theta0 + thp
+    p = p_a * (rho * R * theta / p_a) ** gamma
+    vel = (u, v, w)
+    X = (x, y, z)
+    S = [-sum(sp.diff(rho * vel[c], X[c]) for c in range(3))]
+    for c in range(3):
+        S.append(-sum(vel[d] * sp.diff(vel[c], X[d]) for d in range(3)) - sp.diff(p, X[c]) / rho)
+    S.append(-sum(vel[d] * sp.diff(theta, X[d]) for d in range(3)))
+    fq = sp.lambdify((x, y, z), [rhop, u, v, w, thp], "numpy")
+    fS = sp.lambdify((x, y, z), S, "numpy")
+    return fq, fS
+
+
+def _mms_error(N, ne, perturb, fq, fS, L):
+    mesh = inputs.box_mesh(N, ne, ne, ne, (L, L, L), perturb=perturb, seed=77,
+                           periodic=(True, True, True))
+    rho0, theta0 = inputs.reference_uniform(mesh.xyz[2], 1.2, 300.0)
+    q = np.stack([np.broadcast_to(a, rho0.shape) for a in fq(*mesh.xyz)]).astype(float)
+    Sx = np.stack([np.broadcast_to(a, rho0.shape) for a in fS(*mesh.xyz)]).astype(float)
+    o = orc.Oracle(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc,
+                   np.stack((rho0, theta0)), dict(C, g=0.0))
+    r = o.rhs(q)
+    err = [math.sqrt(np.sum(o.wJ * (r[m] - Sx[m]) ** 2) / np.sum(o.wJ * Sx[m] ** 2))
+           for m in range(5)]
+    return np.array(err)
+
+
+def test_P11_manufactured_solution_convergence_order():
+    """RHS error ~ h^N on 4^3 -> 8^3 -> 16^3 elements (N = 4), uniform and perturbed mesh."""
+    L = 1000.0
+    fq, fS = _manufactured(L)
+    for perturb in (0.0, 0.05):
+        e = [_mms_error(4, ne, perturb, fq, fS, L) for ne in (4, 8, 16)]
+        s1 = np.log2(e[0] / e[1]); s2 = np.log2(e[1] / e[2])
+        assert np.all(e[2] < 2e-4), e[2]
+        assert np.all(s2 > 3.7) and np.all(s2 < 4.3), (perturb, s1, s2)
+
+
+def test_P11_spectral_decay_with_order():
+    """On a fixed 3^3 mesh the error falls super-algebraically with N = 2..8."""
+    L = 1000.0
+    fq, fS = _manufactured(L)
+    errs = np.array([_mms_error(N, 3, 0.05, fq, fS, L).max() for N in range(2, 9)])
+    assert np.all(errs[1:] < 0.7 * errs[:-1]), errs
+    assert errs[-1] < 2e-4 * errs[0], errs
+    assert errs[-1] < 1e-4
+
+
+def test_P13_linear_acoustics_sound_speed():
+    """g = 0, uniform background at rest, tiny plane pressure pulse: the linearisation of
+    Eq. 1 + Eq. 3 gives d2 rho'/dt2 = c^2 d2 rho'/dx2 with c^2 = gamma R T = gamma p0/rho0.
+    For rho' = eps rho0 sin(kx), theta' = 0, u = 0:  d u/dt = -c^2 k eps cos(kx)  (isentropic
+    p' = c^2 rho').  Fixes the EOS linkage, gamma, and the sign of the pressure-gradient term."""
+    N, L = 6, 1000.0
+    mesh = inputs.box_mesh(N, 4, 1, 1, (L, L / 4, L / 4), periodic=(True, True, True))
+    rho0, theta0 = inputs.reference_uniform(mesh.xyz[2], 1.2, 300.0)
+    eps, k = 1e-7, 2 * np.pi / L
+    q = np.zeros((5,) + rho0.shape)
+    q[0] = eps * 1.2 * np.sin(k * mesh.xyz[0])
+    o = orc.Oracle(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc,
+                   np.stack((rho0, theta0)), dict(C, g=0.0))
+    r = o.rhs(q)
+    gamma = C["c_p"] / C["c_v"]
+    p0 = C["p_a"] * (1.2 * C["R_gas"] * 300.0 / C["p_a"]) ** gamma
+    c2 = gamma * p0 / 1.2
+    assert abs(math.sqrt(c2) - 347.0) < 5.0  # ~ speed of sound at ~290 K
+    expect = -c2 * k * eps * np.cos(k * mesh.xyz[0])
+    assert np.max(np.abs(r[1] - expect)) < 1e-4 * np.max(np.abs(expect))
+    assert np.max(np.abs(r[2])) < 1e-12 and np.max(np.abs(r[3])) < 1e-12
+
+
+def test_eos_stable_form_matches_eq3_in_high_precision():
+    """p' of the oracle (log1p/expm1 form, Q6) equals Eq. 3 evaluated with 40
+    digits: checked through the w-momentum tendency of a single affine element at rest,
+    where S_w = -(1/rho) dp'/dz - (rho'/rho) g and everything else vanishes."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    N = 4
+    mesh = inputs.box_mesh(N, 1, 1, 1, (10.0, 10.0, 10.0))
+    z = mesh.xyz[2]
+    rho0 = 1.1 - 1e-3 * z
+    theta0 = 300.0 + 0.01 * z
+    rhop = 1e-4 * (z / 10.0) ** 2
+    thp = 0.3 * (z / 10.0)
+    q = np.zeros((5,) + z.shape); q[0] = rhop; q[4] = thp
+    met, _, _ = orc.metrics(N, mesh.xyz)
+    par = np.array([C["g"], C["p_a"], C["R_gas"], C["c_p"], C["c_v"]])
+    S = orc.tendency(N, par, q, np.stack((rho0, theta0)), met)
+    # high-precision nodal p' then the same spectral derivative in z (2/h * D along zeta)
+    gamma = mp.mpf(C["c_p"]) / mp.mpf(C["c_v"])
+    def pprime(r0, t0, rp, tp):
+        r0, t0, rp, tp = map(mp.mpf, (float(r0), float(t0), float(rp), float(tp)))
+        pa, R = mp.mpf(C["p_a"]), mp.mpf(C["R_gas"])
+        return pa * ((r0 + rp) * R * (t0 + tp) / pa) ** gamma - pa * (r0 * R * t0 / pa) ** gamma
+    Nq = N + 1
+    col = [n * Nq * Nq for n in range(Nq)]  # nodes (0,0,k)
+    pcol = [pprime(rho0[0, n], theta0[0, n], rhop[0, n], thp[0, n]) for n in col]
+    D = orc.dmat(N)
+    for kk in range(Nq):
+        dpdz = sum(mp.mpf(float(D[kk, l])) * pcol[l] for l in range(Nq)) * mp.mpf(2) / mp.mpf(10)
+        n = col[kk]
+        rho = mp.mpf(float(rho0[0, n])) + mp.mpf(float(rhop[0, n]))
+        want = -dpdz / rho - mp.mpf(float(rhop[0, n])) / rho * mp.mpf(C["g"])
+        assert abs(mp.mpf(float(S[3][0, n])) - want) < mp.mpf(2e-12) * abs(want) + mp.mpf(1e-13)
+
+
+# ---------------------------------------------------------------------------------------
+def _kron_reference(mesh, ref, q, const):
+    """P16: brute-force NumPy restatement of A2-A7 with dense Kronecker operators and an
+    explicit boolean scatter matrix; D built here from Lagrange polynomials via np.poly."""
+    N, Nq = mesh.N, mesh.N + 1
+    xi = inputs.lgl_points(N)
+    D = np.empty((Nq, Nq))
+    for l in range(Nq):
+        others = np.delete(xi, l)
+        D[:, l] = np.polyval(np.polyder(np.poly(others) / np.prod(xi[l] - others)), xi)
+    # leg weights by solving the moment equations (exact for degree <= N)
+    V = np.vander(xi, Nq, increasing=True).T
+    mom = np.array([(1 - (-1) ** (p + 1)) / (p + 1) for p in range(Nq)])
+    w = np.linalg.solve(V, mom)
+    I = np.eye(Nq)
+    Dxi = np.kron(I, np.kron(I, D))     # n = i + Nq (j + Nq k): i fastest
+    Deta = np.kron(I, np.kron(D, I))
+    Dzeta = np.kron(D, np.kron(I, I))
+    W = np.kron(w, np.kron(w, w))
+    Ne = mesh.n_elem
+    NL = mesh.n_local
+    S = np.zeros((5, Ne, Nq ** 3)); wJ = np.zeros((Ne, Nq ** 3))
+    g, p_a, R, gamma = const["g"], const["p_a"], const["R_gas"], const["c_p"] / const["c_v"]
+    for e in range(Ne):
+        X = mesh.xyz[:, e, :]
+        Jm = np.stack([np.stack([Dop @ X[c] for Dop in (Dxi, Deta, Dzeta)], axis=-1)
+                       for c in range(3)], axis=-2)          # [n][c][a] = dx_c/dxi_a
+        Ji = np.linalg.inv(Jm)                               # [n][a][c] = dxi_a/dx_c
+        wJ[e] = W * np.linalg.det(Jm)
+        grad = lambda f: np.einsum("na,nac->nc", np.stack([Dxi @ f, Deta @ f, Dzeta @ f], -1), Ji)
+        rho0, th0 = ref[0, e], ref[1, e]
+        rhop, u, v, wv, thp = (q[m, e] for m in range(5))
+        rho = rho0 + rhop
+        pp = p_a * (rho * R * (th0 + thp) / p_a) ** gamma - p_a * (rho0 * R * th0 / p_a) ** gamma
+        vel = np.stack((u, v, wv), -1)
+        S[0, e] = -sum(grad(rho * vel[:, c])[:, c] for c in range(3))
+        gp = grad(pp)
+        for c in range(3):
+            S[1 + c, e] = -np.einsum("nc,nc->n", vel, grad(vel[:, c])) - gp[:, c] / rho
+        S[3, e] -= rhop / rho * g
+        S[4, e] = -np.einsum("nc,nc->n", vel, grad(th0 + thp))
+    Q = np.zeros((NL, mesh.n_global)); Q[np.arange(NL), mesh.intma_cg.ravel()] = 1.0
+    M = Q.T @ wJ.ravel()
+    r = np.stack([(Q @ ((Q.T @ (wJ.ravel() * S[m].ravel())) / M)).reshape(Ne, -1) for m in range(5)])
+    return r
+
+
+@pytest.mark.parametrize("N,periodic", [(2, (False, False, False)), (3, (True, True, False))])
+def test_P16_kronecker_bruteforce(N, periodic):
+    mesh = inputs.box_mesh(N, 2, 2, 2, (200.0, 200.0, 100.0), perturb=0.08, seed=31,
+                           periodic=periodic)
+    rho0, theta0 = inputs.reference_stable(mesh.xyz[2], N_bv=0.02)
+    q = inputs.smooth_random_state(mesh, rho0, theta0, seed=8)
+    ref = np.stack((rho0, theta0))
+    o = orc.Oracle(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, C)
+    got = o.rhs_local(q)
+    o.dss(got)
+    want = _kron_reference(mesh, ref, q, C)
+    for m in range(5):
+        # the brute force uses Eq. 3 literally (p - p0 by subtraction: ~1e-11 Pa of
+        # cancellation noise), hence the looser bound on the momentum rows
+        tol = 1e-7 if 1 <= m <= 3 else 1e-11
+        assert np.linalg.norm(got[m] - want[m]) < tol * np.linalg.norm(want[m]), m
