@@ -1,0 +1,171 @@
+/*
+ * numa_b200.h -- C ABI of libnuma_b200.so
+ *
+ * B200 (sm_100a) implementation of the data-parallel hot path of the xNUMA nonhydrostatic
+ * atmospheric model of arXiv 2504.08157: the matrix-free continuous-Galerkin spectral-
+ * element right-hand side of the compressible Euler equations in the paper's Section-2
+ * form, q = (rho', u, v, w, theta') (Eq. 1a-1c; equation of state Eq. 3,
+ * L76-L80; discretisation Eq. 4-12), its global assembly (DSS; Eq. 10-12,
+ * Alg. 3) and the explicit Runge-Kutta stage update that consumes it
+ * ("updating the state vector", L172).  FP64 throughout (L322).
+ *
+ * Conventions
+ *   Nq = N+1 points per direction, Mn = Nq^3 nodes per element, Ne elements,
+ *   NL = Ne*Mn local (element-duplicated) nodes, local node n = i + Nq*(j + Nq*k)
+ *   (i along xi fastest), faces 0..5 = xi-, xi+, eta-, eta+, zeta-, zeta+.
+ *   Every field is element-local structure-of-arrays:  f[m][e][n]  -- the paper's
+ *   q_e(i,j,k,e,m) (Alg. 1); state variable order m = rho', u, v, w, theta'.
+ *
+ * Pointers
+ *   Unless a function name ends in _host, every array pointer is a DEVICE pointer
+ *   (>= 8-byte aligned; 16-byte alignment enables the vectorised paths) and stays
+ *   caller-owned.  The library allocates no device memory: persistent tables live in the
+ *   caller-provided workspace handed to numa_init_geometry.  `stream` is a cudaStream_t
+ *   passed as void* (NULL = legacy default stream).  All calls except numa_init_geometry
+ *   and the *_host calls only enqueue work on `stream` and return without synchronising.
+ *
+ * Errors
+ *   Every call returns a numa_status; nothing throws.  Argument checks are synchronous and
+ *   happen before any launch.  CUDA launch errors map to NUMA_ERR_CUDA; text in
+ *   numa_last_error().  There is no CPU fallback: without a CUDA device every entry point
+ *   that would launch returns NUMA_ERR_CUDA.
+ */
+#ifndef NUMA_B200_H
+#define NUMA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct numa_ctx numa_ctx; /* opaque; created by numa_init_geometry, freed by numa_destroy */
+
+typedef enum {
+    NUMA_OK = 0,
+    NUMA_ERR_ARG = 1,          /* NULL pointer, N out of range, bad size                     */
+    NUMA_ERR_UNSUPPORTED = 2,  /* method = DG / eqn_set = conservative (not built) */
+    NUMA_ERR_CUDA = 3,         /* CUDA runtime or launch error, or no device                 */
+    NUMA_ERR_NEG_JACOBIAN = 4, /* some node has det(dx/dxi) <= 0                             */
+    NUMA_ERR_WORKSPACE = 5     /* workspace too small or misaligned                          */
+} numa_status;
+
+typedef struct {
+    int32_t N;       /* polynomial order, 2..8 (Eq. 4-5)                            */
+    int32_t method;  /* 0 = CG + DSS (built); 1 = DG face flux -> NUMA_ERR_UNSUPPORTED       */
+    int32_t eqn_set; /* 0 = Eq. 1 (rho',u,v,w,theta'); 1 = conservative -> UNSUPPORTED       */
+    int32_t reserved;
+    int64_t n_elem;   /* Ne                                                                  */
+    int64_t n_global; /* number of unique CG nodes = max(intma_cg)+1 (N_p of Eq. 9)    */
+    double g;         /* gravitational acceleration, Eq. 1b                                  */
+    double p_a;       /* surface pressure of Eq. 3                                           */
+    double R_gas;     /* specific gas constant of dry air, Eq. 3                             */
+    double c_p, c_v;  /* gamma = c_p / c_v, Eq. 3                                            */
+    double f_cor;     /* f-plane Coriolis parameter (BASELINE.json config 3; Q10)  */
+} numa_params;
+
+/* Bytes of device workspace numa_init_geometry needs for these parameters (0 on bad input). */
+size_t numa_workspace_bytes(const numa_params *p);
+
+/* Bytes of device scratch numa_step_rk3 needs (two state-sized buffers: stage state and
+ * assembled tendency). */
+size_t numa_step_scratch_bytes(const numa_params *p);
+
+/*
+ * A0 -- setup ("the simulation is set up ... all data is transferred").
+ * Computes, into the workspace: the LGL derivative matrix D and weights (Eq. 5, Eq. 8);
+ * metric terms grad xi_a and the Jacobian from the nodal coordinates (L92, L149); the
+ * diagonal mass M = DSS(w J) (Eq. 10) and the assembly weight omega = wJ / M
+ * (Eq. 11-12); the node -> copies lists of the deterministic DSS; the background pressure
+ * p0 = p_a (rho0 R theta0 / p_a)^gamma (Eq. 3); copies of ref, sponge and face_bc.
+ *
+ *   xyz       [3][Ne][Mn]  nodal coordinates
+ *   intma_cg  [Ne][Mn]     unique CG node id of every local node (Alg. 3)
+ *   face_bc   [Ne][6]      0 = interior/periodic face, 1 = no-flux wall (L256)
+ *   ref       [2][Ne][Mn]  rho0, theta0 (reference state, L66)
+ *   sponge    [Ne][Mn]     Rayleigh coefficient beta [1/s], or NULL (Q9)
+ *   workspace              >= numa_workspace_bytes(p) bytes, 256-byte aligned
+ *
+ * All inputs may be freed after the call returns (this call synchronises `stream`).
+ * Returns NUMA_ERR_NEG_JACOBIAN if any node has J <= 0.
+ */
+numa_status numa_init_geometry(const numa_params *p, const double *xyz, const int32_t *intma_cg,
+                               const uint8_t *face_bc, const double *ref, const double *sponge,
+                               void *workspace, size_t workspace_bytes, void *stream,
+                               numa_ctx **out);
+
+/*
+ * A2-A6 -- element-local volume term (Alg. 1 kernels 2-4, L207-L222; Alg. 2):
+ * rhs[m][e][n] = omega * S_m(q), S the right-hand side of Eq. 1 with H = 0: tensor-product
+ * LGL derivatives along xi, eta, zeta of p', u, v, w, theta (gradient) and of rho*u
+ * (divergence), chain rule with the metric terms, gravity, times wJ/M (Eq. 11-12).
+ * q, rhs: [5][Ne][Mn]; rhs must not alias q.
+ */
+numa_status numa_rhs(numa_ctx *ctx, const double *q, double *rhs, void *stream);
+
+/*
+ * A7 -- global assembly.  CG: direct stiffness summation (Eq. 10-11; Alg. 3 gather L263-L270
+ * + scatter L283-L291) in place on rhs[5][Ne][Mn]: every local copy of a global node
+ * receives the sum over all copies, accumulated in ascending local-index order (bitwise
+ * reproducible; no floating-point atomics).  DG face flux: NUMA_ERR_UNSUPPORTED.
+ */
+numa_status numa_dss_or_flux(numa_ctx *ctx, double *rhs, void *stream);
+
+/*
+ * A8-A9 -- pointwise sources on the assembled tendency, then the no-flux walls, in place:
+ *   rhs_theta += heating (S_theta of Eq. 1c; [Ne][Mn] K/s or NULL);
+ *   rhs_u += f v, rhs_v -= f u (Coriolis);  rhs_m -= beta q_m, m = u,v,w,theta' (sponge);
+ *   at nodes of wall faces: rhs_vel -= (rhs_vel . n) n per wall face, faces in order 0..5,
+ *   n = outward unit normal -+ grad xi_a / |grad xi_a|  (L256; Q8).
+ */
+numa_status numa_apply_sources(numa_ctx *ctx, const double *q, const double *heating, double *rhs,
+                               void *stream);
+
+/*
+ * A10 -- explicit Runge-Kutta stage update (L172): q_out = a0*q0 + a1*qs + b_dt*rhs over the
+ * 5 fields.  q_out may alias q0 or qs.
+ */
+numa_status numa_rk_stage(numa_ctx *ctx, double a0, double a1, double b_dt, const double *q0,
+                          const double *qs, const double *rhs, double *q_out, void *stream);
+
+/*
+ * A11 -- n_steps SSP-RK3 (Shu-Osher) steps of size dt, in place on q[5][Ne][Mn], through the
+ * fused kernels (same mathematics as numa_rhs -> numa_dss_or_flux -> numa_apply_sources ->
+ * numa_rk_stage per stage; both routes are parity-tested).  heating may be NULL.
+ * scratch: >= numa_step_scratch_bytes(p) bytes, 256-byte aligned.
+ */
+numa_status numa_step_rk3(numa_ctx *ctx, double *q, void *scratch, const double *heating,
+                          double dt, int32_t n_steps, void *stream);
+
+/*
+ * End-to-end variant with HOST buffers: copies q (and heating, if non-NULL) host -> device
+ * into caller-provided device staging buffers, runs n_steps of numa_step_rk3, copies q back
+ * and synchronises.  q_host [5][Ne][Mn] (in/out), heating_host [Ne][Mn] or NULL; pinned host
+ * memory gives the best copy rate.  d_q: device [5][Ne][Mn]; d_heating: device [Ne][Mn] or
+ * NULL iff heating_host is NULL.
+ */
+numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heating_host,
+                               double *d_q, double *d_heating, void *scratch, double dt,
+                               int32_t n_steps, void *stream);
+
+/*
+ * Copies one of the tables built by A0 out of the workspace (device -> device, enqueued on
+ * `stream`), for parity tests of the setup: which = 0 met[9][NL] (d xi_a/d x_c, index
+ * 3a+c), 1 omega[NL], 2 p0[NL], 3 D[Nq*Nq] (D[i*Nq+l] = h_l'(xi_i)), 4 w[Nq].
+ */
+numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, double *out, void *stream);
+
+/* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
+int64_t numa_launch_count(const numa_ctx *ctx);
+
+numa_status numa_destroy(numa_ctx *ctx);
+
+/* Text of the last error of this context ("" if none).  ctx may be NULL: returns the text
+ * of the last error raised without a context (e.g. inside numa_init_geometry). */
+const char *numa_last_error(const numa_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NUMA_B200_H */

@@ -1,0 +1,223 @@
+"""Thin Python binding of libnuma_b200.so (include/numa_b200.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing (and cannot
+be built) or no CUDA device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+_LIB = None
+
+STATUS = {0: "NUMA_OK", 1: "NUMA_ERR_ARG", 2: "NUMA_ERR_UNSUPPORTED", 3: "NUMA_ERR_CUDA",
+          4: "NUMA_ERR_NEG_JACOBIAN", 5: "NUMA_ERR_WORKSPACE"}
+
+EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometry", "numa_rhs",
+           "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
+           "numa_step_rk3_host", "numa_copy_table", "numa_launch_count", "numa_destroy",
+           "numa_last_error"]
+
+
+class NumaParams(C.Structure):
+    _fields_ = [("N", C.c_int32), ("method", C.c_int32), ("eqn_set", C.c_int32),
+                ("reserved", C.c_int32), ("n_elem", C.c_int64), ("n_global", C.c_int64),
+                ("g", C.c_double), ("p_a", C.c_double), ("R_gas", C.c_double),
+                ("c_p", C.c_double), ("c_v", C.c_double), ("f_cor", C.c_double)]
+
+
+class NumaError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("%s: %s" % (STATUS.get(status, status), text))
+        self.status = status
+
+
+def load_library(path: str | None = None):
+    """dlopen libnuma_b200.so (building it in-tree first if it is stale or absent)."""
+    global _LIB
+    if _LIB is not None and path is None:
+        return _LIB
+    libpath = path or _build.LIB
+    if path is None and (not os.path.exists(libpath) or os.environ.get("NUMA_B200_REBUILD")):
+        libpath = _build.build()
+    if not os.path.exists(libpath):
+        raise ImportError("libnuma_b200.so is missing and could not be built; there is no "
+                          "fallback path (run python -m paper_2504_08157_b200.build)")
+    L = C.CDLL(libpath)
+    vp, dp = C.c_void_p, C.c_void_p
+    L.numa_workspace_bytes.argtypes = [C.POINTER(NumaParams)]
+    L.numa_workspace_bytes.restype = C.c_size_t
+    L.numa_step_scratch_bytes.argtypes = [C.POINTER(NumaParams)]
+    L.numa_step_scratch_bytes.restype = C.c_size_t
+    L.numa_init_geometry.argtypes = [C.POINTER(NumaParams), dp, dp, dp, dp, dp, vp, C.c_size_t,
+                                     vp, C.POINTER(vp)]
+    L.numa_rhs.argtypes = [vp, dp, dp, vp]
+    L.numa_dss_or_flux.argtypes = [vp, dp, vp]
+    L.numa_apply_sources.argtypes = [vp, dp, dp, dp, vp]
+    L.numa_rk_stage.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp, vp]
+    L.numa_step_rk3.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
+    L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
+    L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
+    L.numa_launch_count.argtypes = [vp]
+    L.numa_launch_count.restype = C.c_int64
+    L.numa_destroy.argtypes = [vp]
+    L.numa_last_error.argtypes = [vp]
+    L.numa_last_error.restype = C.c_char_p
+    for f in ("numa_init_geometry", "numa_rhs", "numa_dss_or_flux", "numa_apply_sources",
+              "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_host", "numa_copy_table",
+              "numa_destroy"):
+        getattr(L, f).restype = C.c_int
+    if path is None:
+        _LIB = L
+    return L
+
+
+def make_params(N, n_elem, n_global, constants, f_cor=0.0, method=0, eqn_set=0) -> NumaParams:
+    return NumaParams(N=N, method=method, eqn_set=eqn_set, reserved=0, n_elem=n_elem,
+                      n_global=n_global, g=constants["g"], p_a=constants["p_a"],
+                      R_gas=constants["R_gas"], c_p=constants["c_p"], c_v=constants["c_v"],
+                      f_cor=f_cor)
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(a, dtype, device):
+    """numpy array / torch tensor -> contiguous device tensor of the given dtype."""
+    if a is None:
+        return None
+    t = torch.as_tensor(a)
+    return t.to(device=device, dtype=dtype).contiguous()
+
+
+class Numa:
+    """One numa_ctx plus the torch tensors (workspace, scratch) that back it.
+
+    Methods mirror the C ABI one to one: rhs, dss_or_flux, apply_sources, rk_stage,
+    step_rk3, step_rk3_host.  Arrays are torch CUDA float64 tensors [5][Ne][Mn] / [Ne][Mn].
+    """
+
+    def __init__(self, N, xyz, intma_cg, n_global, face_bc, ref, constants, f_cor=0.0,
+                 sponge=None, device="cuda:0", method=0, eqn_set=0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2504_08157_b200 needs a CUDA device; there is no CPU fallback")
+        self.lib = load_library()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        xyz_d = _dev(xyz, torch.float64, self.device)
+        self.n_elem = int(xyz_d.shape[1])
+        self.Mn = (N + 1) ** 3
+        self.N = N
+        self.NL = self.n_elem * self.Mn
+        self.params = make_params(N, self.n_elem, int(n_global), constants, f_cor, method, eqn_set)
+        cg_d = _dev(intma_cg, torch.int32, self.device)
+        bc_d = _dev(face_bc, torch.uint8, self.device)
+        ref_d = _dev(ref, torch.float64, self.device)
+        sp_d = _dev(sponge, torch.float64, self.device)
+        nbytes = self.lib.numa_workspace_bytes(C.byref(self.params))
+        if nbytes == 0 and method == 0 and eqn_set == 0:
+            raise NumaError(1, "numa_workspace_bytes: parameters out of range")
+        self.workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=self.device)
+        self._scratch = None
+        self.ctx = C.c_void_p()
+        st = self.lib.numa_init_geometry(C.byref(self.params), _ptr(xyz_d), _ptr(cg_d), _ptr(bc_d),
+                                         _ptr(ref_d), _ptr(sp_d), _ptr(self.workspace),
+                                         self.workspace.numel(), _stream(), C.byref(self.ctx))
+        if st != 0:
+            raise NumaError(st, self.lib.numa_last_error(None).decode())
+
+    @classmethod
+    def from_workload(cls, wl, device="cuda:0"):
+        m = wl.mesh
+        return cls(m.N, m.xyz, m.intma_cg, m.n_global, m.face_bc, wl.ref, wl.constants,
+                   f_cor=wl.f_cor, sponge=wl.sponge, device=device)
+
+    # -- helpers ------------------------------------------------------------------------
+    def _check(self, st):
+        if st != 0:
+            raise NumaError(st, self.lib.numa_last_error(self.ctx).decode())
+
+    def state(self, a):
+        """Host array -> device state tensor [5][Ne][Mn]."""
+        return _dev(a, torch.float64, self.device)
+
+    def scratch(self):
+        if self._scratch is None:
+            n = self.lib.numa_step_scratch_bytes(C.byref(self.params))
+            self._scratch = torch.empty(n, dtype=torch.uint8, device=self.device)
+        return self._scratch
+
+    def table(self, which):
+        """Copy of a table built by A0: 0 met[9][NL], 1 omega[NL], 2 p0[NL], 3 D[Nq*Nq], 4 w[Nq]."""
+        Nq = self.N + 1
+        n = {0: 9 * self.NL, 1: self.NL, 2: self.NL, 3: Nq * Nq, 4: Nq}[which]
+        out = torch.empty(n, dtype=torch.float64, device=self.device)
+        self._check(self.lib.numa_copy_table(self.ctx, which, _ptr(out), _stream()))
+        return out
+
+    # -- the C ABI ------------------------------------------------------------------------
+    def rhs(self, q, out=None):
+        out = torch.empty_like(q) if out is None else out
+        self._check(self.lib.numa_rhs(self.ctx, _ptr(q), _ptr(out), _stream()))
+        return out
+
+    def dss_or_flux(self, r):
+        self._check(self.lib.numa_dss_or_flux(self.ctx, _ptr(r), _stream()))
+        return r
+
+    def apply_sources(self, q, heating, r):
+        self._check(self.lib.numa_apply_sources(self.ctx, _ptr(q), _ptr(heating), _ptr(r), _stream()))
+        return r
+
+    def rk_stage(self, a0, a1, b_dt, q0, qs, r, out):
+        self._check(self.lib.numa_rk_stage(self.ctx, a0, a1, b_dt, _ptr(q0), _ptr(qs), _ptr(r),
+                                           _ptr(out), _stream()))
+        return out
+
+    def step_rk3(self, q, dt, heating=None, n_steps=1):
+        self._check(self.lib.numa_step_rk3(self.ctx, _ptr(q), _ptr(self.scratch()), _ptr(heating),
+                                           dt, n_steps, _stream()))
+        return q
+
+    def step_rk3_host(self, q_host, dt, heating_host=None, n_steps=1, d_q=None, d_heating=None):
+        """q_host / heating_host: (pinned) CPU float64 tensors; staged through d_q / d_heating."""
+        if d_q is None:
+            d_q = torch.empty(q_host.shape, dtype=torch.float64, device=self.device)
+        if heating_host is not None and d_heating is None:
+            d_heating = torch.empty(heating_host.shape, dtype=torch.float64, device=self.device)
+        self._check(self.lib.numa_step_rk3_host(self.ctx, _ptr(q_host), _ptr(heating_host),
+                                                _ptr(d_q), _ptr(d_heating), _ptr(self.scratch()),
+                                                dt, n_steps, _stream()))
+        return q_host
+
+    def full_rhs(self, q, heating=None):
+        """Convenience: the four separate calls that form L(q)."""
+        r = self.rhs(q)
+        self.dss_or_flux(r)
+        self.apply_sources(q, heating, r)
+        return r
+
+    @property
+    def launch_count(self):
+        return int(self.lib.numa_launch_count(self.ctx))
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None and self.ctx.value:
+            self.lib.numa_destroy(self.ctx)
+            self.ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

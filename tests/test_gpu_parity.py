@@ -1,0 +1,316 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU
+oracle on the same seeded inputs, element by element.
+
+Tolerances (BASELINE.json north_star): relative L2 <= 1e-12 per field per RHS call and
+<= 1e-10 per field after 100 RK3 steps.  DESIGN.md "Tolerance" (reading Q19): when a field
+of the oracle is (nearly) zero by cancellation, the error is measured against the norm of
+T = sum of |terms| of that equation instead (both are reported in the assertion message).
+Index work (DSS gather/scatter order) is compared bit-exactly.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2504_08157_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS = 1e-12
+TOL_100 = 1e-10
+
+
+def rel_l2(g, o, T=None, floor=1e-3):
+    """Per-field relative L2 error.  If T is given and ||o|| < floor*||T|| (the field is small
+    by cancellation) the error is taken relative to ||T|| (Q19)."""
+    out = []
+    for m in range(o.shape[0]):
+        no = np.linalg.norm(o[m])
+        den = no
+        if T is not None:
+            nT = np.linalg.norm(T[m])
+            if no < floor * nT:
+                den = nT
+        err = np.linalg.norm(g[m] - o[m])
+        out.append(err / den if den > 0 else err)
+    return np.array(out)
+
+
+def _pair(wl):
+    o = orc.Oracle.from_workload(wl)
+    g = binding.Numa.from_workload(wl)
+    return o, g
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _assembled_T(o, q):
+    """Assembled sum-of-|terms| used to scale ill-conditioned fields."""
+    r, T = o.rhs_local(q, want_T=True)
+    o.dss(T)
+    return T
+
+
+CASES = [
+    # (config, N, scale)
+    (1, 4, 1.0), (1, 2, 1.0), (1, 3, 1.0), (1, 5, 1.0), (1, 6, 1.0), (1, 7, 1.0), (1, 8, 1.0),
+    (2, 4, 0.35), (2, 7, 0.25),
+    (3, 4, 0.07), (4, 3, 0.05), (4, 5, 0.06), (4, 6, 0.06), (4, 8, 0.07), (5, 7, 0.03),
+]
+
+
+@pytest.mark.parametrize("cfg,N,scale", CASES)
+def test_setup_tables_match_oracle(cfg, N, scale):
+    wl = inputs.make_workload(cfg, N=N, scale=scale)
+    o, g = _pair(wl)
+    D = _np(g.table(3)).reshape(N + 1, N + 1)
+    w = _np(g.table(4))
+    xi_o, w_o = orc.lgl(N)
+    assert np.max(np.abs(D - orc.dmat(N))) < 2e-13
+    assert np.max(np.abs(w - w_o)) < 1e-15
+    met = _np(g.table(0)).reshape(o.met.shape)
+    for c in range(9):
+        scale_c = np.max(np.abs(o.met[3 * (c // 3):3 * (c // 3) + 3]))
+        assert np.max(np.abs(met[c] - o.met[c])) < 1e-12 * scale_c, c
+    om = _np(g.table(1)).reshape(o.omega.shape)
+    assert np.max(np.abs(om - o.omega)) < 1e-12
+    p0 = _np(g.table(2)).reshape(o.omega.shape)
+    c = wl.constants
+    p0_o = c["p_a"] * (wl.ref[0] * c["R_gas"] * wl.ref[1] / c["p_a"]) ** (c["c_p"] / c["c_v"])
+    assert np.max(np.abs(p0 / p0_o - 1.0)) < 1e-14
+
+
+@pytest.mark.parametrize("cfg,N,scale", CASES)
+def test_rhs_call_by_call_parity_on_generic_state(cfg, N, scale):
+    """numa_rhs, numa_dss_or_flux, numa_apply_sources each against the oracle, on a seeded
+    smooth state with all five fields non-zero (parity protocol)."""
+    wl = inputs.make_workload(cfg, N=N, scale=scale)
+    o, g = _pair(wl)
+    q = inputs.smooth_random_state(wl.mesh, wl.ref[0], wl.ref[1], seed=1234 + cfg)
+    qd = g.state(q)
+    hd = None if wl.heating is None else g.state(wl.heating)
+    # A2-A6
+    r_o, T = o.rhs_local(q, want_T=True)
+    r_g = g.rhs(qd)
+    e = rel_l2(_np(r_g), r_o, T)
+    assert np.all(e <= TOL_RHS), ("numa_rhs", e)
+    # A7 on the GPU's own local result: bit-exact against the oracle's DSS of the same data
+    r_in = _np(r_g).copy()
+    g.dss_or_flux(r_g)
+    want = o.dss(r_in.copy())
+    assert np.array_equal(_np(r_g), want), "numa_dss_or_flux is not bit-exact"
+    # full chain
+    o.dss(r_o); o.dss(T)
+    e = rel_l2(_np(r_g), r_o, T)
+    assert np.all(e <= TOL_RHS), ("after DSS", e)
+    g.apply_sources(qd, hd, r_g)
+    o.apply_sources(q, wl.heating, r_o)
+    e = rel_l2(_np(r_g), r_o, T)
+    assert np.all(e <= TOL_RHS), ("after sources", e)
+    # walls: no normal component left
+    if o.wall_node.size:
+        rv = _np(r_g).reshape(5, -1)[1:4][:, o.wall_node]
+        scale_v = np.max(np.abs(rv)) + 1e-300
+        assert np.max(np.abs(np.einsum("ct,tc->t", rv, o.wall_normal))) < 1e-13 * scale_v
+
+
+@pytest.mark.parametrize("cfg,N,scale", [(1, 4, 1.0), (2, 4, 0.35), (3, 4, 0.07), (5, 7, 0.03)])
+def test_rhs_parity_on_workload_state_after_10_steps(cfg, N, scale):
+    wl = inputs.make_workload(cfg, N=N, scale=scale)
+    o, g = _pair(wl)
+    q = wl.q
+    for _ in range(10):
+        q = o.step_rk3(q, wl.dt, wl.heating)
+    r_o = o.rhs(q, wl.heating)
+    T = _assembled_T(o, q)
+    hd = None if wl.heating is None else g.state(wl.heating)
+    r_g = g.full_rhs(g.state(q), hd)
+    e = rel_l2(_np(r_g), r_o, T)
+    assert np.all(e <= TOL_RHS), e
+
+
+def test_sources_and_rk_stage_pointwise():
+    wl = inputs.make_workload(3, scale=0.05)
+    o, g = _pair(wl)
+    rng = np.random.default_rng(3)
+    q = inputs.smooth_random_state(wl.mesh, wl.ref[0], wl.ref[1], seed=9)
+    r = rng.standard_normal(q.shape)
+    r_g = g.state(r)
+    g.apply_sources(g.state(q), g.state(wl.heating), r_g)
+    r_o = o.apply_sources(q, wl.heating, r.copy())
+    assert np.max(np.abs(_np(r_g) - r_o)) < 1e-14 * np.max(np.abs(r_o))
+    q0 = rng.standard_normal(q.shape)
+    out = torch.empty_like(r_g)
+    g.rk_stage(0.75, 0.25, 0.25 * 0.1, g.state(q0), g.state(q), g.state(r), out)
+    want = orc.rk_stage(0.75, 0.25, 0.25 * 0.1, q0, q, r)
+    assert np.max(np.abs(_np(out) - want)) <= 4e-16 * np.max(np.abs(want))
+    # aliasing q_out = qs
+    qs_d = g.state(q)
+    g.rk_stage(0.75, 0.25, 0.025, g.state(q0), qs_d, g.state(r), qs_d)
+    assert np.array_equal(_np(qs_d), _np(out))
+
+
+@pytest.mark.parametrize("cfg,N,scale,steps", [(1, 4, 1.0, 100), (2, 4, 0.25, 100), (2, 7, 0.2, 100),
+                                               (3, 4, 0.06, 100), (5, 7, 0.025, 50)])
+def test_100_rk3_steps_parity(cfg, N, scale, steps):
+    """numa_step_rk3 (fused route) and the four-call route against the oracle after `steps`
+    SSP-RK3 steps (config 5 states 50 steps)."""
+    wl = inputs.make_workload(cfg, N=N, scale=scale)
+    o, g = _pair(wl)
+    q = wl.q
+    refresh = wl.heating_refresh_steps
+    heat = wl.heating
+    qd = g.state(wl.q)
+    hd = None if heat is None else g.state(heat)
+    for s in range(steps):
+        if refresh and s > 0 and s % refresh == 0:
+            heat = wl.heating_at(s // refresh)
+            hd = g.state(heat)
+        q = o.step_rk3(q, wl.dt, heat)
+        g.step_rk3(qd, wl.dt, hd, 1)
+    assert np.all(np.isfinite(q))
+    e = rel_l2(_np(qd), q)
+    # fields that are still zero to round-off in the oracle are compared absolutely
+    nz = np.array([np.linalg.norm(q[m]) > 0 for m in range(5)])
+    assert np.all(e[nz] <= TOL_100), e
+    # four separate calls give the same answer as the fused route after 3 steps
+    qa = g.state(wl.q); qb = g.state(wl.q)
+    hd0 = None if wl.heating is None else g.state(wl.heating)
+    g.step_rk3(qa, wl.dt, hd0, 3)
+    q1 = torch.empty_like(qb)
+    (s1, s2, s3), dt = orc.SSP_RK3, wl.dt
+    for _ in range(3):
+        g.rk_stage(s1[0], s1[1], s1[2] * dt, qb, qb, g.full_rhs(qb, hd0), q1)
+        g.rk_stage(s2[0], s2[1], s2[2] * dt, qb, q1, g.full_rhs(q1, hd0), q1)
+        g.rk_stage(s3[0], s3[1], s3[2] * dt, qb, q1, g.full_rhs(q1, hd0), qb)
+    e2 = rel_l2(_np(qa), _np(qb))
+    assert np.all(e2 <= 1e-13), e2
+
+
+def test_bitwise_reproducible_run_to_run():
+    wl = inputs.make_workload(2, scale=0.3)
+    g = binding.Numa.from_workload(wl)
+    a = g.state(wl.q); b = g.state(wl.q)
+    g.step_rk3(a, wl.dt, None, 5)
+    g.step_rk3(b, wl.dt, None, 5)
+    assert torch.equal(a, b)
+    g2 = binding.Numa.from_workload(wl)
+    c = g2.state(wl.q)
+    g2.step_rk3(c, wl.dt, None, 5)
+    assert torch.equal(a, c)
+
+
+def test_copies_of_a_global_node_stay_bitwise_equal():
+    wl = inputs.make_workload(1)
+    g = binding.Numa.from_workload(wl)
+    q = g.state(wl.q)
+    g.step_rk3(q, wl.dt, None, 4)
+    qh = _np(q).reshape(5, -1)
+    cg = wl.mesh.intma_cg.ravel()
+    for m in (0, 4):  # fields without wall projection
+        glob = np.zeros(wl.mesh.n_global); glob[cg] = qh[m]
+        assert np.array_equal(glob[cg], qh[m])
+
+
+def test_atmosphere_at_rest_stays_bitwise_at_rest_on_gpu():
+    for cfg, scale in ((1, 1.0), (3, 0.05)):
+        wl = inputs.make_workload(cfg, scale=scale)
+        g = binding.Numa.from_workload(wl)
+        q = torch.zeros(wl.q.shape, dtype=torch.float64, device="cuda")
+        r = g.full_rhs(q, None)
+        assert torch.all(r == 0)
+        g.step_rk3(q, wl.dt, None, 3)
+        assert torch.all(q == 0)
+
+
+# ---------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [2, 3, 4])
+def test_single_element_and_ragged_element_counts(N):
+    """One element (no shared nodes at all) and element counts that are not a multiple of
+    the elements-per-block of the kernels."""
+    for dims in ((1, 1, 1), (3, 1, 1), (5, 3, 1), (7, 1, 3)):
+        mesh = inputs.box_mesh(N, *dims, (100.0 * dims[0], 100.0 * dims[1], 100.0 * dims[2]),
+                               perturb=0.05, seed=N)
+        rho0, theta0 = inputs.reference_neutral(mesh.xyz[2])
+        ref = np.stack((rho0, theta0))
+        q = inputs.smooth_random_state(mesh, rho0, theta0, seed=2)
+        o = orc.Oracle(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+        g = binding.Numa(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+        r_o, T = o.rhs_local(q, want_T=True)
+        o.dss(r_o); o.dss(T); o.apply_sources(q, None, r_o)
+        r_g = g.full_rhs(g.state(q), None)
+        e = rel_l2(_np(r_g), r_o, T)
+        assert np.all(e <= TOL_RHS), (dims, e)
+        qd = g.state(q)
+        g.step_rk3(qd, 0.01, None, 2)
+        qo = o.step_rk3(o.step_rk3(q, 0.01), 0.01)
+        assert np.all(rel_l2(_np(qd), qo) <= 1e-13)
+
+
+def test_periodic_mesh_parity():
+    N = 4
+    mesh = inputs.box_mesh(N, 4, 3, 3, (400.0, 300.0, 300.0), perturb=0.05, seed=8,
+                           periodic=(True, True, False))
+    rho0, theta0 = inputs.reference_neutral(mesh.xyz[2])
+    ref = np.stack((rho0, theta0))
+    q = inputs.smooth_random_state(mesh, rho0, theta0, seed=2)
+    o = orc.Oracle(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    g = binding.Numa(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    r_o, T = o.rhs_local(q, want_T=True)
+    o.dss(r_o); o.dss(T); o.apply_sources(q, None, r_o)
+    e = rel_l2(_np(g.full_rhs(g.state(q), None)), r_o, T)
+    assert np.all(e <= TOL_RHS), e
+
+
+def test_scrambled_global_numbering_and_unused_ids():
+    """The library must not rely on any structure of intma_cg: random relabelling of the
+    global ids with gaps (unused ids) gives the same assembled result."""
+    N = 3
+    mesh = inputs.box_mesh(N, 3, 3, 2, (300.0, 300.0, 200.0), perturb=0.05, seed=8)
+    rho0, theta0 = inputs.reference_neutral(mesh.xyz[2])
+    ref = np.stack((rho0, theta0))
+    q = inputs.smooth_random_state(mesh, rho0, theta0, seed=2)
+    rng = np.random.default_rng(0)
+    perm = rng.permutation(2 * mesh.n_global)[:mesh.n_global].astype(np.int32)
+    cg2 = perm[mesh.intma_cg]
+    g1 = binding.Numa(N, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    g2 = binding.Numa(N, mesh.xyz, cg2, 2 * mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    r1 = g1.full_rhs(g1.state(q), None)
+    r2 = g2.full_rhs(g2.state(q), None)
+    assert torch.equal(r1, r2)
+
+
+def test_init_errors_on_device():
+    mesh = inputs.box_mesh(2, 2, 1, 1, (2.0, 1.0, 1.0))
+    rho0, theta0 = inputs.reference_neutral(mesh.xyz[2])
+    ref = np.stack((rho0, theta0))
+    xyz = mesh.xyz.copy(); xyz[0] = -xyz[0]
+    with pytest.raises(binding.NumaError) as ei:
+        binding.Numa(2, xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    assert ei.value.status == 4
+    with pytest.raises(binding.NumaError) as ei:
+        binding.Numa(2, mesh.xyz, mesh.intma_cg, mesh.n_global - 1, mesh.face_bc, ref, inputs.CONSTANTS)
+    assert ei.value.status == 1
+    with pytest.raises(binding.NumaError) as ei:
+        binding.Numa(2, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS,
+                     method=1)
+    assert ei.value.status == 2
+    g = binding.Numa(2, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    q = g.state(np.zeros((5,) + rho0.shape))
+    with pytest.raises(binding.NumaError):
+        g.rhs(q, out=q)  # rhs must not alias q
+
+
+def test_host_buffer_entry_point_matches_device_path():
+    wl = inputs.make_workload(3, scale=0.05)
+    g = binding.Numa.from_workload(wl)
+    qd = g.state(wl.q); hd = g.state(wl.heating)
+    g.step_rk3(qd, wl.dt, hd, 2)
+    qh = torch.from_numpy(wl.q.copy()).pin_memory()
+    hh = torch.from_numpy(wl.heating.copy()).pin_memory()
+    g.step_rk3_host(qh, wl.dt, hh, 2)
+    assert torch.equal(qh, qd.cpu())
