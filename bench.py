@@ -1,0 +1,352 @@
+#!/usr/bin/env python
+"""Benchmark of the hot path: SSP-RK3 steps of the matrix-free CG
+Euler RHS + stage update on a synthetic limited-area tropical-cyclone workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg2|cfg2n7|cfg4nX|cfg5]
+                    [--impl reference]
+
+One "step" = one SSP-RK3 time step = 3 passes of the whole hot path (rows A2-A10 of SURVEY.md
+8(a): volume RHS, DSS, sources + walls, RK stage update).  The metric is BASELINE.json's:
+FP64 nodal RHS evaluations per second per RK stage, in GDOF/s with the paper's DOF = 5 x local
+nodes, i.e. value = 5 * NL * 3 * K / t.  Prints ONE JSON line on rank 0.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded
+sample of the same workload; it is the slow reference arm, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fp64_nodal_rhs_evals_per_s_per_rk_stage"
+UNIT = "GDOF/s"
+
+
+def parse_workload(name):
+    """-> (config, N or None)"""
+    name = name.lower()
+    if name == "cfg2n7":
+        return 2, 7
+    if name.startswith("cfg4n"):
+        return 4, int(name[5:])
+    if name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
+        return int(name[3]), None
+    raise SystemExit("unknown workload %r" % name)
+
+
+def b_alg_bytes(N, has_src):
+    """Algorithmic bytes per local node per RK stage."""
+    f_face = 1.0 - ((N - 1.0) / (N + 1.0)) ** 3
+    n_src = 2 if has_src else 0
+    return 8.0 * (5 + 5 * (2.0 / 3.0) + 9 + 1 + 2 + n_src + 5) + 2 * 8 * 5 * f_face
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [p.strip() for p in r.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax = float(parts[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def cpu_sample_workload(config, N):
+    """Bounded sample of the workload for the oracle: same physics and element shapes, fewer
+    element columns (about 1 M local nodes, i.e. seconds per RK3 step on a few cores)."""
+    from paper_2504_08157_b200 import inputs
+    if config in (1, 2):
+        wl = inputs.make_workload(config, N=N)
+        return wl, "whole workload %s (%d local nodes)" % (wl.name, wl.mesh.n_local)
+    n = N or (7 if config == 5 else 4)
+    nz = 24 if config == 5 else 20
+    base = {3: 100, 4: inputs.CFG4_NXY.get(n, 113), 5: 160}[config]
+    nxy = max(2, int(round((1.0e6 / (n + 1) ** 3 / nz) ** 0.5)))
+    wl = inputs.make_workload(config, N=N, scale=min(1.0, nxy / base))
+    return wl, "%s: %dx%dx%d elements (%d local nodes), same physics and element heights" % (
+        wl.name, wl.mesh.nx, wl.mesh.ny, wl.mesh.nz, wl.mesh.n_local)
+
+
+def time_oracle(wl, steps, warmup):
+    from oracle import oracle as orc
+    o = orc.Oracle.from_workload(wl)
+    q = wl.q
+    for _ in range(warmup):
+        q = o.step_rk3(q, wl.dt, wl.heating)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        q = o.step_rk3(q, wl.dt, wl.heating)
+    t = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    cores = min(cores, os.cpu_count() or cores)
+    return t, cores
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on a bounded sample (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    config, N = parse_workload(args.workload)
+    wl, sample = cpu_sample_workload(config, N)
+    steps = max(1, min(args.steps, 5))
+    warm = max(0, min(args.warmup, 1))
+    t, cores = time_oracle(wl, steps, warm)
+    NL = wl.mesh.n_local
+    value = 5.0 * NL * 3 * steps / t / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": 1e3 * t / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "sample_of": args.workload, "N": wl.mesh.N,
+                   "local_nodes": NL, "integrator": "SSP-RK3", "dt": wl.dt},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2504_08157_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference "
+                         "for the CPU oracle arm")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    config, N = parse_workload(args.workload)
+    wl = inputs.make_workload(config, N=N)
+    mesh = wl.mesh
+    NL = mesh.n_local
+    g = binding.Numa.from_workload(wl, device=str(dev))
+    q = g.state(wl.q)
+    heat = None if wl.heating is None else g.state(wl.heating)
+    g.scratch()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------
+    g.step_rk3(q, wl.dt, heat, args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    g.profile(True)
+    l0 = g.launch_count
+    ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    g.step_rk3(q, wl.dt, heat, args.steps)
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = g.launch_count - l0
+    prof = g.profile_read()
+    g.profile(False)
+    clocks = sampler.stop() if rank == 0 else None
+    finite = bool(torch.isfinite(q).all().item())
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- end to end through the C ABI with host buffers ---------------------------------
+    qh = torch.from_numpy(wl.q.copy()).pin_memory()
+    hh = None if wl.heating is None else torch.from_numpy(wl.heating.copy()).pin_memory()
+    dq = torch.empty_like(q)
+    dh = None if heat is None else torch.empty_like(heat)
+    e2e_steps = max(1, min(args.steps, 10))
+    g.step_rk3_host(qh, wl.dt, hh, 1, dq, dh)   # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        g.step_rk3_host(qh, wl.dt, hh, 1, dq, dh)   # H2D state+heating, 1 step, D2H state, sync
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        t_e2e = float(t.item())
+    h2d = 5 * NL * 8 + (NL * 8 if hh is not None else 0)
+    d2h = 5 * NL * 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    dof_evals = 5.0 * NL * 3 * args.steps * world
+    value = dof_evals / (ms * 1e-3) / 1e9
+    e2e_value = 5.0 * NL * 3 * e2e_steps * world / t_e2e / 1e9
+
+    # ---- roofline of the dominant kernel -------------------------------------------------
+    peak, peak_src = measured_peaks()
+    has_src = wl.heating is not None
+    balg = b_alg_bytes(mesh.N, has_src)
+    roofline = None
+    if prof:
+        dom = max(prof.items(), key=lambda kv: kv[1][0])
+        dom_ms, dom_n = dom[1]
+        # B_alg covers one whole stage (all kernels of a stage); the dominant kernel's own
+        # algorithmic share is reported as `kernel_bytes_per_node`.
+        kb = kernel_alg_bytes(dom[0], mesh.N, has_src)
+        achieved = kb * NL / (dom_ms / dom_n * 1e-3) / 1e9
+        stage_ms = ms / (3 * args.steps)
+        roofline = {
+            "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "traffic": None, "kernel": dom[0],
+            "kernel_ms": dom_ms / dom_n, "kernel_share_of_step": dom_ms / ms,
+            "kernel_bytes_per_node": kb, "peak_source": peak_src,
+            "stage": {"b_alg_bytes_per_node": balg, "ms": stage_ms,
+                      "achieved": balg * NL / (stage_ms * 1e-3) / 1e9,
+                      "frac": balg * NL / (stage_ms * 1e-3) / 1e9 / peak},
+            "kernels": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
+                            "share_of_step": v[0] / ms} for k, v in prof.items()},
+        }
+
+    # ---- CPU baseline: the oracle on a bounded sample ------------------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        swl, sample = cpu_sample_workload(config, N)
+        t_cpu, cores = time_oracle(swl, 2, 1)
+        cpu = {"value": 5.0 * swl.mesh.n_local * 3 * 2 / t_cpu / 1e9, "unit": UNIT, "cores": cores,
+               "kind": "oracle", "sample": sample + ", 2 RK3 steps after 1 warm-up"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "N": mesh.N, "elements": [mesh.nx, mesh.ny, mesh.nz],
+                   "local_nodes": NL, "integrator": "SSP-RK3 (3 RHS + 3 stage updates per step)",
+                   "dt": wl.dt, "multi_gpu": "replicas only" if world > 1 else "single",
+                   "l2": "inputs larger than L2" if 22 * NL * 8 > 4 * 126e6 else
+                         "working set may be L2-resident (reported, not a roofline case)",
+                   "finite": finite},
+        "gnode_per_s": value / 5.0,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                "call": "numa_step_rk3_host (pinned host buffers)"},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def kernel_alg_bytes(name, N, has_src):
+    """Algorithmic bytes per local node per launch of one kernel."""
+    f_face = 1.0 - ((N - 1.0) / (N + 1.0)) ** 3
+    n_src = 2 if has_src else 0
+    if name.startswith("k_rhs"):
+        return 8.0 * (5 + 9 + 1 + 3 + 5)              # q, met, omega, ref3 in; rhs out
+    if name.startswith("k_dss"):
+        return 2 * 8.0 * 5 * f_face                   # face nodes read + written
+    if name.startswith("k_sources"):
+        return 8.0 * (4 + n_src + 4 + 4)              # u,v,w,theta', heat, beta, rhs in/out (4 fields)
+    if name.startswith("k_rk"):
+        return 8.0 * (5 + 5 * (2.0 / 3.0) + 5 + 5)    # q0 (2/3 of stages), qs, rhs in; q out
+    if name.startswith("k_stage_volume"):
+        return 8.0 * (5 + 5 * (2.0 / 3.0) + 9 + 1 + 3 + n_src + 5)
+    if name.startswith("k_stage_dss"):
+        return 2 * 8.0 * 5 * f_face
+    return 0.0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="numa_b200", choices=["numa_b200", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl != "reference":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

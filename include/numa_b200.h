@@ -156,6 +156,18 @@ numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heat
  */
 numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, double *out, void *stream);
 
+/*
+ * Optional per-kernel timing with CUDA events recorded on the launching stream around every
+ * kernel this context launches (bench.py's roofline figure).  numa_profile_enable(ctx, 1)
+ * clears the accumulators and starts recording, (ctx, 0) stops.  numa_profile_read waits for
+ * the recorded events and returns the accumulated device time and launch count of one
+ * kernel id: 0 volume (numa_rhs), 1 DSS, 2 sources, 3 RK stage, 4 fused stage volume,
+ * 5 fused stage DSS.  numa_kernel_name gives a printable name.
+ */
+numa_status numa_profile_enable(numa_ctx *ctx, int32_t enable);
+numa_status numa_profile_read(numa_ctx *ctx, int32_t kernel_id, double *total_ms, int64_t *launches);
+const char *numa_kernel_name(int32_t kernel_id);
+
 /* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
 int64_t numa_launch_count(const numa_ctx *ctx);
 

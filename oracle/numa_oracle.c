@@ -113,6 +113,18 @@ void orc_dmat(int N, const double *xi, double *D)
  * element:  f_xi(i,j,k) = sum_l D[i][l] f(l,j,k), f_eta = sum_l D[j][l] f(i,l,k),
  * f_zeta = sum_l D[k][l] f(i,j,l).  hold1/2/3 of the listing are fx/fe/fz.
  * ---------------------------------------------------------------------------------- */
+static void ref_derivs_abs(int Nq, const double *D, const double *f, int i, int j, int k,
+                           double *fx, double *fe, double *fz)
+{
+    double a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    for (int l = 0; l < Nq; ++l) {
+        a1 += fabs(D[i * Nq + l] * f[NODE(l, j, k)]);
+        a2 += fabs(D[j * Nq + l] * f[NODE(i, l, k)]);
+        a3 += fabs(D[k * Nq + l] * f[NODE(i, j, l)]);
+    }
+    *fx = a1; *fe = a2; *fz = a3;
+}
+
 static void ref_derivs(int Nq, const double *D, const double *f, int i, int j, int k,
                        double *fx, double *fe, double *fz)
 {
@@ -125,10 +137,29 @@ static void ref_derivs(int Nq, const double *D, const double *f, int i, int j, i
     *fx = hold1; *fe = hold2; *fz = hold3;
 }
 
+/* Alg. 2 in difference form (see orc_metrics): sum_{l != i} D[i][l] (f_l - f_i). */
+static void ref_derivs_diff(int Nq, const double *D, const double *f, int i, int j, int k,
+                            double *fx, double *fe, double *fz)
+{
+    double hold1 = 0.0, hold2 = 0.0, hold3 = 0.0, f0 = f[NODE(i, j, k)];
+    for (int l = 0; l < Nq; ++l) {
+        if (l != i) hold1 = hold1 + D[i * Nq + l] * (f[NODE(l, j, k)] - f0);
+        if (l != j) hold2 = hold2 + D[j * Nq + l] * (f[NODE(i, l, k)] - f0);
+        if (l != k) hold3 = hold3 + D[k * Nq + l] * (f[NODE(i, j, l)] - f0);
+    }
+    *fx = hold1; *fe = hold2; *fz = hold3;
+}
+
 /* ------------------------------------------------------------------------------------
  * A0.2  Metric terms ("mapped ... via metric terms", L149 J = dx/dxi of the
  * isoparametric mapping; formula per DESIGN.md Q4): differentiate the nodal coordinates
  * with D, J = det(dx/dxi), grad xi_a = rows of the inverse (cross products / J).
+ * The coordinate derivatives are evaluated in difference form,
+ *   x_xi(i,j,k) = sum_{l != i} D[i][l] (x(l,j,k) - x(i,j,k)),
+ * which is Alg. 2's sum with the diagonal entry D[i][i] = -sum_{l != i} D[i][l] written out
+ * (identical in exact arithmetic).  A coordinate that is constant along a reference
+ * direction then has an exactly zero derivative, and the round-off is relative to the
+ * element size instead of to the distance from the origin (Q4).
  * Returns the number of nodes with J <= 0.
  * ---------------------------------------------------------------------------------- */
 long orc_metrics(int N, long Ne, const double *xyz, double *met, double *jac)
@@ -146,9 +177,9 @@ long orc_metrics(int N, long Ne, const double *xyz, double *met, double *jac)
             for (int j = 0; j < Nq; ++j)
                 for (int i = 0; i < Nq; ++i) {
                     double xx, xe, xz, yx, ye, yz, zx, ze, zz;
-                    ref_derivs(Nq, D, x, i, j, k, &xx, &xe, &xz);
-                    ref_derivs(Nq, D, y, i, j, k, &yx, &ye, &yz);
-                    ref_derivs(Nq, D, z, i, j, k, &zx, &ze, &zz);
+                    ref_derivs_diff(Nq, D, x, i, j, k, &xx, &xe, &xz);
+                    ref_derivs_diff(Nq, D, y, i, j, k, &yx, &ye, &yz);
+                    ref_derivs_diff(Nq, D, z, i, j, k, &zx, &ze, &zz);
                     /* J = x_xi . (x_eta x x_zeta) */
                     double c0 = ye * zz - yz * ze, c1 = xz * ze - xe * zz, c2 = xe * yz - xz * ye;
                     double J = xx * c0 + yx * c1 + zx * c2;
@@ -249,7 +280,8 @@ long orc_wall_list(int N, long Ne, const uint8_t *face_bc, const double *met,
  *       p' = p0 * expm1( gamma * ( log1p(rho'/rho0) + log1p(theta'/theta0) ) )
  *   gradient (Alg. 2) of the five variables (p', u, v, w, theta)  (L424); theta is
  *       differentiated as theta' plus theta0 separately, grad theta = grad theta' +
- *       grad theta0, both with the same D (Q7)
+ *       grad theta0, both with the same D, theta0 taken relative to its value at the
+ *       element's first node (D annihilates the constant; Q7)
  *   chain rule: d f/d x_c = sum_a f_{xi_a} d xi_a/d x_c                  (Q2)
  *   divergence of the momentum F = rho u only (L424): 9 reference derivatives
  *   Eq. 1a:  S_rho   = - div F
@@ -257,8 +289,10 @@ long orc_wall_list(int N, long Ne, const uint8_t *face_bc, const double *met,
  *   Eq. 1c:  S_theta = - u.grad(theta0 + theta')
  *
  * par = {g, p_a, R_gas, c_p, c_v}.  T (optional, may be NULL) receives, per equation and
- * node, the sum of the absolute values of the terms added to form S (used only to scale
- * parity errors of ill-conditioned fields, Q19).
+ * node, the same expression evaluated with every product and every contraction term
+ * replaced by its absolute value (sum_l |D f_l| etc.): the quantity that bounds the
+ * rounding error of ANY evaluation order, |fl(S) - S| <= c eps T.  It is used only to
+ * scale parity errors of fields that are small by cancellation (Q19).
  * ---------------------------------------------------------------------------------- */
 void orc_tendency(int N, long Ne, const double *par, const double *q, const double *ref,
                   const double *met, double *S, double *T)
@@ -272,8 +306,9 @@ void orc_tendency(int N, long Ne, const double *par, const double *q, const doub
     orc_dmat(N, xi, D);
 #pragma omp parallel
     {
-        /* per-element nodal work arrays: pp, u, v, w, th', th0, Fx, Fy, Fz */
-        double *wk = (double *)malloc(sizeof(double) * 9 * Mn);
+        /* per-element nodal work arrays: pp, u, v, w, th', th0, Fx, Fy, Fz (+ |p'| scale for T) */
+        double *wk = (double *)malloc(sizeof(double) * 10 * Mn);
+        double *ppabs = wk + 9 * Mn;
         double *pp = wk, *uu = wk + Mn, *vv = wk + 2 * Mn, *ww = wk + 3 * Mn, *thp = wk + 4 * Mn,
                *th0 = wk + 5 * Mn, *Fx = wk + 6 * Mn, *Fy = wk + 7 * Mn, *Fz = wk + 8 * Mn;
 #pragma omp for schedule(static)
@@ -286,7 +321,9 @@ void orc_tendency(int N, long Ne, const double *par, const double *q, const doub
                 double rho = rho0 + rhop;
                 double p0 = p_a * pow(rho0 * R * theta0 / p_a, gamma);
                 pp[n] = p0 * expm1(gamma * (log1p(rhop / rho0) + log1p(tp / theta0)));
-                uu[n] = u; vv[n] = v; ww[n] = wv; thp[n] = tp; th0[n] = theta0;
+                /* scale of p' for T: p' is itself a sum of two terms that may cancel */
+                ppabs[n] = p0 * gamma * (fabs(log1p(rhop / rho0)) + fabs(log1p(tp / theta0)));
+                uu[n] = u; vv[n] = v; ww[n] = wv; thp[n] = tp; th0[n] = theta0 - ref[1 * NL + b];
                 Fx[n] = rho * u; Fy[n] = rho * v; Fz[n] = rho * wv;
             }
             for (int k = 0; k < Nq; ++k)
@@ -306,13 +343,12 @@ void orc_tendency(int N, long Ne, const double *par, const double *q, const doub
                         }
                         /* divergence of F = rho u */
                         const double *F[3] = {Fx, Fy, Fz};
-                        double div = 0.0, adiv = 0.0;
+                        double div = 0.0;
                         for (int c = 0; c < 3; ++c) {
                             double fx, fe, fz;
                             ref_derivs(Nq, D, F[c], i, j, k, &fx, &fe, &fz);
                             double d = fx * m[0 + c] + fe * m[3 + c] + fz * m[6 + c];
                             div += d;
-                            adiv += fabs(fx * m[0 + c]) + fabs(fe * m[3 + c]) + fabs(fz * m[6 + c]);
                         }
                         double rhop = q[0 * NL + p];
                         double rho = ref[0 * NL + p] + rhop;
@@ -329,17 +365,26 @@ void orc_tendency(int N, long Ne, const double *par, const double *q, const doub
                         S[3 * NL + p] = -advw - grad[0][2] / rho - (rhop / rho) * g;
                         S[4 * NL + p] = -advt;
                         if (T) {
-                            T[0 * NL + p] = adiv;
-                            T[1 * NL + p] = fabs(u * grad[1][0]) + fabs(v * grad[1][1]) +
-                                            fabs(wv * grad[1][2]) + fabs(grad[0][0] / rho);
-                            T[2 * NL + p] = fabs(u * grad[2][0]) + fabs(v * grad[2][1]) +
-                                            fabs(wv * grad[2][2]) + fabs(grad[0][1] / rho);
-                            T[3 * NL + p] = fabs(u * grad[3][0]) + fabs(v * grad[3][1]) +
-                                            fabs(wv * grad[3][2]) + fabs(grad[0][2] / rho) +
-                                            fabs((rhop / rho) * g);
-                            T[4 * NL + p] = fabs(u * grad[4][0]) + fabs(v * grad[4][1]) +
-                                            fabs(wv * grad[4][2]) + fabs(u * grad[5][0]) +
-                                            fabs(v * grad[5][1]) + fabs(wv * grad[5][2]);
+                            double ag[6][3], adv[3] = {fabs(u), fabs(v), fabs(wv)};
+                            for (int f = 0; f < 6; ++f) {
+                                double ax, ae, az;
+                                ref_derivs_abs(Nq, D, f == 0 ? ppabs : fld[f], i, j, k, &ax, &ae, &az);
+                                for (int c = 0; c < 3; ++c)
+                                    ag[f][c] = ax * fabs(m[0 + c]) + ae * fabs(m[3 + c]) + az * fabs(m[6 + c]);
+                            }
+                            double adiv2 = 0.0;
+                            for (int c = 0; c < 3; ++c) {
+                                double ax, ae, az;
+                                ref_derivs_abs(Nq, D, F[c], i, j, k, &ax, &ae, &az);
+                                adiv2 += ax * fabs(m[0 + c]) + ae * fabs(m[3 + c]) + az * fabs(m[6 + c]);
+                            }
+                            T[0 * NL + p] = adiv2;
+                            for (int c = 0; c < 3; ++c)
+                                T[(1 + c) * NL + p] = adv[0] * ag[1 + c][0] + adv[1] * ag[1 + c][1] +
+                                                      adv[2] * ag[1 + c][2] + ag[0][c] / rho;
+                            T[3 * NL + p] += fabs((rhop / rho) * g);
+                            T[4 * NL + p] = adv[0] * (ag[4][0] + ag[5][0]) + adv[1] * (ag[4][1] + ag[5][1]) +
+                                            adv[2] * (ag[4][2] + ag[5][2]);
                         }
                     }
         }

@@ -21,7 +21,7 @@ STATUS = {0: "NUMA_OK", 1: "NUMA_ERR_ARG", 2: "NUMA_ERR_UNSUPPORTED", 3: "NUMA_E
 EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometry", "numa_rhs",
            "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
            "numa_step_rk3_host", "numa_copy_table", "numa_launch_count", "numa_destroy",
-           "numa_last_error"]
+           "numa_last_error", "numa_profile_enable", "numa_profile_read", "numa_kernel_name"]
 
 
 class NumaParams(C.Structure):
@@ -63,6 +63,12 @@ def load_library(path: str | None = None):
     L.numa_step_rk3.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
     L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
+    L.numa_profile_enable.argtypes = [vp, C.c_int32]
+    L.numa_profile_enable.restype = C.c_int
+    L.numa_profile_read.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    L.numa_profile_read.restype = C.c_int
+    L.numa_kernel_name.argtypes = [C.c_int32]
+    L.numa_kernel_name.restype = C.c_char_p
     L.numa_launch_count.argtypes = [vp]
     L.numa_launch_count.restype = C.c_int64
     L.numa_destroy.argtypes = [vp]
@@ -206,6 +212,19 @@ class Numa:
         self.dss_or_flux(r)
         self.apply_sources(q, heating, r)
         return r
+
+    def profile(self, enable=True):
+        self._check(self.lib.numa_profile_enable(self.ctx, 1 if enable else 0))
+
+    def profile_read(self):
+        """{kernel name: (total device ms, launches)} accumulated since profile(True)."""
+        out = {}
+        for kid in range(6):
+            ms = C.c_double(); n = C.c_int64()
+            self._check(self.lib.numa_profile_read(self.ctx, kid, C.byref(ms), C.byref(n)))
+            if n.value:
+                out[self.lib.numa_kernel_name(kid).decode()] = (ms.value, n.value)
+        return out
 
     @property
     def launch_count(self):

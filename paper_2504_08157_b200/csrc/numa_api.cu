@@ -88,8 +88,10 @@ void numa_build_lgl(int N, LglTables *t)
 // ---------------------------------------------------------------------------------------
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
+static const size_t kSmallTmp = (size_t)4 << 20;  // CUB temp storage for small meshes
+
 struct WsLayout {
-    size_t met, omega, ref3, sponge, start, copies, sh_nodes, face_bc, flags, total;
+    size_t met, omega, ref3, sponge, start, copies, sh_nodes, face_bc, flags, small_tmp, total;
     size_t scratch_bytes;  // init-time scratch, aliased onto the (not yet written) met region
 };
 
@@ -114,6 +116,7 @@ static WsLayout ws_layout(const numa_params *p)
     L.sh_nodes = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
     L.face_bc = off; off = align_up(off + (size_t)p->n_elem * 8);
     L.flags = off; off = align_up(off + 64);
+    L.small_tmp = off; off = align_up(off + kSmallTmp);
     L.total = off;
     return L;
 }
@@ -270,7 +273,8 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
         int32_t *valsA = keysB + NL;
         int32_t *valsB = valsA + NL;
         void *cub_tmp = (void *)align_up((size_t)(valsB + NL));
-        size_t cub_avail = (size_t)((ws + L.omega) - (char *)cub_tmp);
+        size_t cub_avail = (char *)cub_tmp < ws + L.omega ? (size_t)((ws + L.omega) - (char *)cub_tmp) : 0;
+        if (cub_avail < kSmallTmp) { cub_tmp = ws + L.small_tmp; cub_avail = kSmallTmp; }
         CK(cudaMemsetAsync(c->d_flags, 0, 64, s));
         k_iota_check<<<grid_for(NL), 256, 0, s>>>(valsA, intma_cg, keysA, NL, NG, c->d_flags);
         CK(cudaGetLastError());
@@ -296,6 +300,7 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
             int32_t *d_num = c->d_flags + 8;
             void *tmp2 = (void *)c->ref3;
             size_t avail2 = (size_t)3 * NL * 8, need2 = 0;
+            if (avail2 < kSmallTmp) { tmp2 = ws + L.small_tmp; avail2 = kSmallTmp; }
             CK(cub::DeviceSelect::If(nullptr, need2, ids, c->sh_nodes, d_num, (int)NG, pred, s));
             if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
             CK(cub::DeviceSelect::If(tmp2, need2, ids, c->sh_nodes, d_num, (int)NG, pred, s));
@@ -448,10 +453,52 @@ extern "C" numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, doubl
     return NUMA_OK;
 }
 
+extern "C" numa_status numa_profile_enable(numa_ctx *ctx, int32_t enable)
+{
+    if (!ctx) return NUMA_ERR_ARG;
+    for (auto &r : ctx->recs) { ctx->pool.push_back(r.a); ctx->pool.push_back(r.b); }
+    ctx->recs.clear();
+    for (int i = 0; i < K_COUNT; ++i) { ctx->prof_ms[i] = 0.0; ctx->prof_n[i] = 0; }
+    ctx->prof = enable != 0;
+    return NUMA_OK;
+}
+
+extern "C" numa_status numa_profile_read(numa_ctx *ctx, int32_t kernel_id, double *total_ms,
+                                         int64_t *launches)
+{
+    if (!ctx || kernel_id < 0 || kernel_id >= K_COUNT || !total_ms || !launches) return NUMA_ERR_ARG;
+    for (auto &r : ctx->recs) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess) {
+            ctx->err = "numa_profile_read: event error";
+            cudaGetLastError();
+            return NUMA_ERR_CUDA;
+        }
+        ctx->prof_ms[r.id] += ms;
+        ctx->prof_n[r.id] += 1;
+        ctx->pool.push_back(r.a); ctx->pool.push_back(r.b);
+    }
+    ctx->recs.clear();
+    *total_ms = ctx->prof_ms[kernel_id];
+    *launches = ctx->prof_n[kernel_id];
+    return NUMA_OK;
+}
+
+extern "C" const char *numa_kernel_name(int32_t kernel_id)
+{
+    static const char *names[K_COUNT] = {"k_rhs (volume)", "k_dss", "k_sources", "k_rk",
+                                         "k_stage_volume (fused)", "k_stage_dss (fused)"};
+    return (kernel_id >= 0 && kernel_id < K_COUNT) ? names[kernel_id] : "";
+}
+
 extern "C" int64_t numa_launch_count(const numa_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" numa_status numa_destroy(numa_ctx *ctx)
 {
+    if (ctx) {
+        for (auto &r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+        for (auto &e : ctx->pool) cudaEventDestroy(e);
+    }
     delete ctx;
     return NUMA_OK;
 }

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "../../include/numa_b200.h"
 
@@ -14,6 +15,11 @@ struct LglTables {
     double D[NUMA_MAX_NQ * NUMA_MAX_NQ];  // D[i*Nq + l] = h_l'(xi_i)  (Alg. 2)
     double w[NUMA_MAX_NQ];                // quadrature weights (Eq. 8)
 };
+
+// kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
+enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_COUNT = 6 };
+
+struct ProfRec { int id; cudaEvent_t a, b; };
 
 struct numa_ctx {
     numa_params par;
@@ -35,6 +41,33 @@ struct numa_ctx {
     int has_walls;
     int64_t launches;
     std::string err;
+    // per-kernel event timing
+    bool prof = false;
+    std::vector<ProfRec> recs;
+    std::vector<cudaEvent_t> pool;
+    double prof_ms[K_COUNT] = {0};
+    int64_t prof_n[K_COUNT] = {0};
+};
+
+// RAII: counts the launch and, when profiling is on, brackets it with events on the stream
+struct LaunchScope {
+    numa_ctx *c; int id; cudaStream_t s; cudaEvent_t a = nullptr, b = nullptr;
+    static cudaEvent_t get(numa_ctx *c)
+    {
+        cudaEvent_t e;
+        if (!c->pool.empty()) { e = c->pool.back(); c->pool.pop_back(); return e; }
+        cudaEventCreate(&e);
+        return e;
+    }
+    LaunchScope(numa_ctx *c_, int id_, cudaStream_t s_) : c(c_), id(id_), s(s_)
+    {
+        c->launches++;
+        if (c->prof) { a = get(c); b = get(c); cudaEventRecord(a, s); }
+    }
+    ~LaunchScope()
+    {
+        if (c->prof) { cudaEventRecord(b, s); c->recs.push_back({id, a, b}); }
+    }
 };
 
 // host-side table construction (tables.cpp part of numa_api.cu)

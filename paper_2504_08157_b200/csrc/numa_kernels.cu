@@ -39,6 +39,28 @@ __device__ __forceinline__ void ref_derivs(const double *__restrict__ f, int i, 
     fx = a; fe = b; fz = c;
 }
 
+// Difference form used for the geometry only: sum_{l != i} D[i][l] (f_l - f_i); exact zero
+// for a coordinate that is constant along the direction (Q4).
+template <int Nq>
+__device__ __forceinline__ void ref_derivs_diff(const double *__restrict__ f, int i, int j, int k,
+                                                const double (&Di)[Nq], const double (&Dj)[Nq],
+                                                const double (&Dk)[Nq], double &fx, double &fe,
+                                                double &fz)
+{
+    const double *fi = f + Nq * (j + Nq * k);
+    const double *fj = f + i + Nq * Nq * k;
+    const double *fk = f + i + Nq * j;
+    const double f0 = f[i + Nq * (j + Nq * k)];
+    double a = 0.0, b = 0.0, c = 0.0;
+#pragma unroll
+    for (int l = 0; l < Nq; ++l) {
+        if (l != i) a = fma(Di[l], fi[l] - f0, a);
+        if (l != j) b = fma(Dj[l], fj[l * Nq] - f0, b);
+        if (l != k) c = fma(Dk[l], fk[l * Nq * Nq] - f0, c);
+    }
+    fx = a; fe = b; fz = c;
+}
+
 // Per-node tendency S(q) of Eq. 1 with H = 0, given the element's nodal work arrays in
 // shared memory: sh[0..8] = p', u, v, w, theta', theta0, Fx, Fy, Fz (each Mn doubles).
 // m[9] = d xi_a / d x_c at this node.  Uses the contravariant velocity U^a = u . grad xi_a so
@@ -88,8 +110,9 @@ __device__ __forceinline__ void node_tendency(const double *__restrict__ sh, int
 
 // A2: pointwise pre-pass for one node -> the nine nodal work values.
 __device__ __forceinline__ void node_prepass(double rhop, double u, double v, double w, double thp,
-                                             double rho0, double theta0, double p0, double gamma,
-                                             double *__restrict__ sh, int Mn, int n)
+                                             double rho0, double theta0, double theta0_e0,
+                                             double p0, double gamma, double *__restrict__ sh,
+                                             int Mn, int n)
 {
     // Eq. 3 in cancellation-free form: p' = p0 * expm1(gamma * log1p(x)),
     // 1 + x = (1 + rho'/rho0)(1 + theta'/theta0)   (Q6)
@@ -101,7 +124,7 @@ __device__ __forceinline__ void node_prepass(double rhop, double u, double v, do
     sh[2 * Mn + n] = v;
     sh[3 * Mn + n] = w;
     sh[4 * Mn + n] = thp;
-    sh[5 * Mn + n] = theta0;
+    sh[5 * Mn + n] = theta0 - theta0_e0;  // relative to the element's first node (Q7)
     sh[6 * Mn + n] = rho * u;
     sh[7 * Mn + n] = rho * v;
     sh[8 * Mn + n] = rho * w;
@@ -171,7 +194,7 @@ k_rhs(const double *__restrict__ q, const double *__restrict__ ref3,
         rhop = q[0 * NL + p];
         rho0 = ref3[0 * NL + p];
         node_prepass(rhop, q[1 * NL + p], q[2 * NL + p], q[3 * NL + p], q[4 * NL + p], rho0,
-                     ref3[1 * NL + p], ref3[2 * NL + p], gamma, she, Mn, n);
+                     ref3[1 * NL + p], ref3[1 * NL + e * Mn], ref3[2 * NL + p], gamma, she, Mn, n);
     }
     __syncthreads();
     if (!valid) return;
@@ -291,9 +314,9 @@ k_metrics(const double *__restrict__ xyz, double *__restrict__ met, double *__re
     __syncthreads();
     if (!valid) return;
     double xx, xe, xz, yx, ye, yz, zx, ze, zz;
-    ref_derivs<Nq>(she + 0 * Mn, i, j, k, Di, Dj, Dk, xx, xe, xz);
-    ref_derivs<Nq>(she + 1 * Mn, i, j, k, Di, Dj, Dk, yx, ye, yz);
-    ref_derivs<Nq>(she + 2 * Mn, i, j, k, Di, Dj, Dk, zx, ze, zz);
+    ref_derivs_diff<Nq>(she + 0 * Mn, i, j, k, Di, Dj, Dk, xx, xe, xz);
+    ref_derivs_diff<Nq>(she + 1 * Mn, i, j, k, Di, Dj, Dk, yx, ye, yz);
+    ref_derivs_diff<Nq>(she + 2 * Mn, i, j, k, Di, Dj, Dk, zx, ze, zz);
     const double c0 = ye * zz - yz * ze, c1 = xz * ze - xe * zz, c2 = xe * yz - xz * ye;
     const double J = xx * c0 + yx * c1 + zx * c2;
     if (!(J > 0.0)) atomicOr(flags, 1);
@@ -368,14 +391,14 @@ cudaError_t launch_metrics(numa_ctx *c, const double *xyz, double *wJ_out, cudaS
 
 cudaError_t launch_rhs(numa_ctx *c, const double *q, double *rhs, cudaStream_t s)
 {
-    c->launches++;
+    LaunchScope ls(c, K_VOLUME, s);
     DISPATCH_N(rhs_N, c, q, rhs, s);
 }
 
 cudaError_t launch_dss(numa_ctx *c, double *r, int nfields, cudaStream_t s)
 {
     if (c->n_shared == 0) return cudaSuccess;
-    c->launches++;
+    LaunchScope ls(c, K_DSS, s);
     const int64_t blocks = (c->n_shared + 255) / 256;
     k_dss<<<(unsigned)blocks, 256, 0, s>>>(r, c->sh_nodes, c->dss_start, c->dss_copies,
                                            c->n_shared, c->NL, nfields);
@@ -394,14 +417,14 @@ cudaError_t launch_mass(numa_ctx *c, cudaStream_t s)
 cudaError_t launch_sources(numa_ctx *c, const double *q, const double *heat, double *rhs,
                            cudaStream_t s)
 {
-    c->launches++;
+    LaunchScope ls(c, K_SOURCES, s);
     DISPATCH_N(sources_N, c, q, heat, rhs, s);
 }
 
 cudaError_t launch_rk(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
                       const double *qs, const double *rhs, double *qout, cudaStream_t s)
 {
-    c->launches++;
+    LaunchScope ls(c, K_RK, s);
     const int64_t n = 5 * c->NL;
     int64_t blocks = (n + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;

@@ -147,7 +147,19 @@ def box_mesh(N, nx, ny, nz, extent, origin=(0.0, 0.0, 0.0), z_ratio=1.0, perturb
     # trilinear weights for local node n = i + Nq*(j + Nq*k): W[c][n], c = corner (dx,dy,dz)
     wi = np.stack((a, b))  # [2][Nq]
     xyz = np.empty((3, Ne, Mn))
+    if perturb == 0.0:
+        # separable (axis-aligned) mesh: each coordinate depends on one index only, so that it
+        # is bit-identical along the other two reference directions
+        lx = vx[ex][:, None] * a[None, :] + vx[ex + 1][:, None] * b[None, :]   # [Ne][Nq]
+        ly = vy[ey][:, None] * a[None, :] + vy[ey + 1][:, None] * b[None, :]
+        lz = vz[ez][:, None] * a[None, :] + vz[ez + 1][:, None] * b[None, :]
+        shape = (Ne, Nq, Nq, Nq)
+        xyz[0] = np.broadcast_to(lx[:, None, None, :], shape).reshape(Ne, Mn)
+        xyz[1] = np.broadcast_to(ly[:, None, :, None], shape).reshape(Ne, Mn)
+        xyz[2] = np.broadcast_to(lz[:, :, None, None], shape).reshape(Ne, Mn)
     for comp, V in enumerate((VX, VY, VZ)):
+        if perturb == 0.0:
+            break
         acc = np.zeros((Ne, Nq, Nq, Nq))  # [e][k][j][i]
         for cz in (0, 1):
             for cy in (0, 1):
