@@ -68,8 +68,7 @@ typedef struct {
 /* Bytes of device workspace numa_init_geometry needs for these parameters (0 on bad input). */
 size_t numa_workspace_bytes(const numa_params *p);
 
-/* Bytes of device scratch numa_step_rk3 needs (two state-sized buffers: stage state and
- * assembled tendency). */
+/* Bytes of device scratch numa_step_rk3 needs (one state-sized buffer: the stage state). */
 size_t numa_step_scratch_bytes(const numa_params *p);
 
 /*

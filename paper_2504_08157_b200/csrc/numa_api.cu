@@ -91,7 +91,7 @@ static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a
 static const size_t kSmallTmp = (size_t)4 << 20;  // CUB temp storage for small meshes
 
 struct WsLayout {
-    size_t met, omega, ref3, sponge, start, copies, sh_nodes, face_bc, flags, small_tmp, total;
+    size_t met, omega, ref3, sponge, start, copies, sh_nodes, dss_idx, face_bc, flags, small_tmp, total;
     size_t scratch_bytes;  // init-time scratch, aliased onto the (not yet written) met region
 };
 
@@ -114,6 +114,7 @@ static WsLayout ws_layout(const numa_params *p)
     L.start = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
     L.copies = off; off = align_up(off + NL * 4);
     L.sh_nodes = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
+    L.dss_idx = off; off = align_up(off + NL * 4);
     L.face_bc = off; off = align_up(off + (size_t)p->n_elem * 8);
     L.flags = off; off = align_up(off + 64);
     L.small_tmp = off; off = align_up(off + kSmallTmp);
@@ -131,7 +132,7 @@ extern "C" size_t numa_step_scratch_bytes(const numa_params *p)
 {
     if (!params_ok(p)) return 0;
     const size_t Nq = p->N + 1, NL = (size_t)p->n_elem * Nq * Nq * Nq;
-    return 2 * align_up(5 * NL * 8);
+    return align_up(5 * NL * 8);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -167,6 +168,34 @@ struct SharedPred {
     const int32_t *start;
     __device__ bool operator()(int32_t g) const { return start[g + 1] - start[g] >= 2; }
 };
+
+// sort key of a shared node: (multiplicity class, first copy); class 0,1,2 = 2,4,8 copies,
+// 3 = anything else.  Counts the classes in cnt[0..3].
+__global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *__restrict__ start,
+                             const int32_t *__restrict__ copies, uint64_t *__restrict__ keys,
+                             int64_t n, unsigned long long *cnt)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
+        const int32_t g = nodes[t];
+        const int32_t s = start[g], c = start[g + 1] - s;
+        const uint64_t cls = (c == 2) ? 0 : (c == 4) ? 1 : (c == 8) ? 2 : 3;
+        keys[t] = (cls << 32) | (uint32_t)copies[s];
+        atomicAdd(cnt + cls, 1ULL);
+    }
+}
+
+// transposed copy lists of one class: idx[a*n + t] = a-th copy of the t-th node
+__global__ void k_class_lists(const int32_t *__restrict__ nodes, const int32_t *__restrict__ start,
+                              const int32_t *__restrict__ copies, int32_t *__restrict__ idx,
+                              int64_t n, int C)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
+        const int32_t s = start[nodes[t]];
+        for (int a = 0; a < C; ++a) idx[(int64_t)a * n + t] = copies[s + a];
+    }
+}
 
 __global__ void k_ref3(const double *__restrict__ ref, double *__restrict__ ref3, int64_t NL,
                        double p_a, double R, double gamma)
@@ -261,6 +290,7 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
     c->dss_start = (int32_t *)(ws + L.start);
     c->dss_copies = (int32_t *)(ws + L.copies);
     c->sh_nodes = (int32_t *)(ws + L.sh_nodes);
+    c->dss_idx = (int32_t *)(ws + L.dss_idx);
     c->face_bc = (uint8_t *)(ws + L.face_bc);
     c->d_flags = (int32_t *)(ws + L.flags);
     {
@@ -289,26 +319,70 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
         k_find_starts<<<grid_for(NL), 256, 0, s>>>(dk.Current(), c->dss_start, NL, NG);
         CK(cudaGetLastError());
         CK(cudaMemcpyAsync(c->dss_copies, dv.Current(), NL * 4, cudaMemcpyDeviceToDevice, s));
-        // --- metrics and wJ (wJ parked in `omega`), then omega = wJ / M via the CSR lists.
-        // (the sort scratch aliased `met`; the stream order makes the reuse safe)
-        CK(launch_metrics(c, xyz, c->omega, s));
-        CK(launch_mass(c, s));
-        // --- list of SHARED global nodes (multiplicity >= 2), ascending; CUB temp in `ref3`
+        // --- SHARED global nodes (multiplicity >= 2), sorted by (multiplicity class, first
+        // copy), and the transposed per-class copy lists of the DSS kernel.  Scratch: the part
+        // of the `met` region behind the first sort's buffers.
         {
             SharedPred pred{c->dss_start};
             thrust::counting_iterator<int32_t> ids(0);
             int32_t *d_num = c->d_flags + 8;
-            void *tmp2 = (void *)c->ref3;
-            size_t avail2 = (size_t)3 * NL * 8, need2 = 0;
+            unsigned long long *d_cnt = (unsigned long long *)(c->d_flags + 10);  // 4 counters
+            char *scr2 = (char *)align_up((size_t)(valsB + NL));
+            char *scr_end = ws + L.omega;
+            int32_t *nodesA = (int32_t *)scr2;                         // [NG]
+            int32_t *nodesB = nodesA + NG;                             // [NG]
+            uint64_t *kA = (uint64_t *)align_up((size_t)(nodesB + NG));  // [NG]
+            uint64_t *kB = kA + NG;
+            void *tmp2 = (void *)align_up((size_t)(kB + NG));
+            size_t avail2 = (char *)tmp2 < scr_end ? (size_t)(scr_end - (char *)tmp2) : 0, need2 = 0;
+            if ((char *)tmp2 > scr_end) { errstr = "internal: setup scratch does not fit"; goto cuda_fail; }
             if (avail2 < kSmallTmp) { tmp2 = ws + L.small_tmp; avail2 = kSmallTmp; }
-            CK(cub::DeviceSelect::If(nullptr, need2, ids, c->sh_nodes, d_num, (int)NG, pred, s));
+            CK(cub::DeviceSelect::If(nullptr, need2, ids, nodesA, d_num, (int)NG, pred, s));
             if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
-            CK(cub::DeviceSelect::If(tmp2, need2, ids, c->sh_nodes, d_num, (int)NG, pred, s));
+            CK(cub::DeviceSelect::If(tmp2, need2, ids, nodesA, d_num, (int)NG, pred, s));
             int32_t h_num = 0;
             CK(cudaMemcpyAsync(&h_num, d_num, 4, cudaMemcpyDeviceToHost, s));
             CK(cudaStreamSynchronize(s));
             c->n_shared = h_num;
+            for (int k = 0; k < 3; ++k) { c->cls_n[k] = 0; c->cls_base[k] = 0; }
+            c->n_gen = 0;
+            c->gen_nodes = c->sh_nodes;
+            if (h_num > 0) {
+                k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, c->dss_start, c->dss_copies, kA,
+                                                            h_num, d_cnt);
+                CK(cudaGetLastError());
+                cub::DoubleBuffer<uint64_t> dk2(kA, kB);
+                cub::DoubleBuffer<int32_t> dv2(nodesA, nodesB);
+                CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, dk2, dv2, h_num, 0, 34, s));
+                if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
+                CK(cub::DeviceRadixSort::SortPairs(tmp2, need2, dk2, dv2, h_num, 0, 34, s));
+                CK(cudaMemcpyAsync(c->sh_nodes, dv2.Current(), (size_t)h_num * 4, cudaMemcpyDeviceToDevice, s));
+                unsigned long long h_cnt[4] = {0, 0, 0, 0};
+                CK(cudaMemcpyAsync(h_cnt, d_cnt, 32, cudaMemcpyDeviceToHost, s));
+                CK(cudaStreamSynchronize(s));
+                int64_t node_off = 0, idx_off = 0;
+                for (int k = 0; k < 3; ++k) {
+                    const int C = 2 << k;
+                    c->cls_n[k] = (int64_t)h_cnt[k];
+                    c->cls_base[k] = idx_off;
+                    if (c->cls_n[k] > 0) {
+                        k_class_lists<<<grid_for(c->cls_n[k]), 256, 0, s>>>(
+                            c->sh_nodes + node_off, c->dss_start, c->dss_copies, c->dss_idx + idx_off,
+                            c->cls_n[k], C);
+                        CK(cudaGetLastError());
+                    }
+                    node_off += c->cls_n[k];
+                    idx_off += c->cls_n[k] * C;
+                }
+                c->gen_nodes = c->sh_nodes + node_off;
+                c->n_gen = (int64_t)h_cnt[3];
+                c->launches += 6;
+            }
         }
+        // --- metrics and wJ (wJ parked in `omega`), then omega = wJ / M via the CSR lists.
+        // (the setup scratch aliased `met`; the stream order makes the reuse safe)
+        CK(launch_metrics(c, xyz, c->omega, s));
+        CK(launch_mass(c, s));
         k_ref3<<<grid_for(NL), 256, 0, s>>>(ref, c->ref3, NL, p->p_a, p->R_gas, c->gamma);
         CK(cudaGetLastError());
         if (sponge) CK(cudaMemcpyAsync(c->sponge, sponge, NL * 8, cudaMemcpyDeviceToDevice, s));
@@ -368,7 +442,7 @@ extern "C" numa_status numa_dss_or_flux(numa_ctx *ctx, double *rhs, void *stream
 {
     if (!ctx || !rhs) return arg_fail(ctx, "numa_dss_or_flux: NULL argument");
     if (ctx->par.method != 0) { ctx->err = "DG face flux is not built"; return NUMA_ERR_UNSUPPORTED; }
-    CKC(launch_dss(ctx, rhs, 5, (cudaStream_t)stream));
+    CKC(launch_dss_classes(ctx, rhs, K_DSS, (cudaStream_t)stream));
     return NUMA_OK;
 }
 
@@ -398,19 +472,17 @@ extern "C" numa_status numa_step_rk3(numa_ctx *ctx, double *q, void *scratch, co
     if (!ctx || !q || !scratch) return arg_fail(ctx, "numa_step_rk3: NULL argument");
     if (n_steps < 0 || ((uintptr_t)scratch & 255)) return arg_fail(ctx, "numa_step_rk3: bad n_steps or scratch alignment");
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t half = numa_step_scratch_bytes(&ctx->par) / 2;
     double *q1 = (double *)scratch;
-    double *r = (double *)((char *)scratch + half);
     for (int step = 0; step < n_steps; ++step) {
         // stage 1: q1 = q + dt L(q);  stage 2: q1 = 3/4 q + 1/4 q1 + 1/4 dt L(q1);
-        // stage 3: q  = 1/3 q + 2/3 q1 + 2/3 dt L(q1)
+        // stage 3: q  = 1/3 q + 2/3 q1 + 2/3 dt L(q1).  Each stage: the volume kernel writes the
+        // update as DSS partial sums (element-local, so q_out may alias qs or q0), then the DSS
+        // completes the shared nodes in place.
         for (int st = 0; st < 3; ++st) {
             const double *qs = (st == 0) ? q : q1;
             double *qo = (st == 2) ? q : q1;
-            CKC(launch_rhs(ctx, qs, r, s));
-            CKC(launch_dss(ctx, r, 5, s));
-            CKC(launch_sources(ctx, qs, heating, r, s));
-            CKC(launch_rk(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, q, qs, r, qo, s));
+            CKC(launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, q, qs, heating, qo, s));
+            CKC(launch_dss_classes(ctx, qo, K_FUSED_DSS, s));
         }
     }
     return NUMA_OK;

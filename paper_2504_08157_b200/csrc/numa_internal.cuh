@@ -36,6 +36,13 @@ struct numa_ctx {
     int32_t *dss_copies;  // [NL]    local indices, ascending within a node
     int32_t *sh_nodes;    // [n_shared] global ids of SHARED nodes (multiplicity >= 2), ascending
     int64_t n_shared;
+    // the same lists by multiplicity class C = 2, 4, 8, transposed: dss_idx[base + a*n + t] is
+    // copy a of the t-th node of the class (nodes ordered by their first copy); nodes of any
+    // other multiplicity >= 2 go through the CSR lists (gen_nodes)
+    int32_t *dss_idx;     // [<= NL]
+    int64_t cls_n[3], cls_base[3];
+    int32_t *gen_nodes;   // [n_gen] (tail of the sorted shared-node list)
+    int64_t n_gen;
     uint8_t *face_bc;     // [Ne][8] (padded to 8 bytes per element)
     int32_t *d_flags;     // [4] device error flags
     int has_walls;
@@ -77,12 +84,37 @@ void numa_build_lgl(int N, LglTables *t);
 cudaError_t launch_metrics(numa_ctx *c, const double *xyz, double *wJ_out, cudaStream_t s);
 cudaError_t launch_mass(numa_ctx *c, cudaStream_t s);
 cudaError_t launch_rhs(numa_ctx *c, const double *q, double *rhs, cudaStream_t s);
-cudaError_t launch_dss(numa_ctx *c, double *r, int nfields, cudaStream_t s);
 cudaError_t launch_sources(numa_ctx *c, const double *q, const double *heat, double *rhs,
                            cudaStream_t s);
 cudaError_t launch_rk(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
                       const double *qs, const double *rhs, double *qout, cudaStream_t s);
-// fused stage: volume + sources + walls + RK written as partial sums, then in-place DSS
-cudaError_t launch_stage_fused(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
-                               const double *qs, const double *heat, double *qout,
-                               cudaStream_t s);
+// fused stage (numa_stage.cu): volume + sources + walls + RK written as DSS partial sums,
+// then the in-place DSS by multiplicity class (kernel_id = profiling slot)
+cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
+                                const double *qs, const double *heat, double *qout,
+                                cudaStream_t s);
+cudaError_t launch_dss_classes(numa_ctx *c, double *r, int kernel_id, cudaStream_t s);
+
+#ifdef __CUDACC__
+// No-flux wall projection at one node (A9): faces in order 0..5; n = -+ grad xi_a/|grad xi_a|.
+template <int Nq>
+__device__ __forceinline__ void wall_project(const uint8_t *__restrict__ bc, int i, int j, int k,
+                                             const double (&m)[9], double &ru, double &rv,
+                                             double &rw)
+{
+    const int idx[3] = {i, j, k};
+#pragma unroll
+    for (int f = 0; f < 6; ++f) {
+        const int a = f >> 1;
+        const bool on = bc[f] && (idx[a] == ((f & 1) ? (Nq - 1) : 0));
+        if (on) {
+            const double gx = m[3 * a + 0], gy = m[3 * a + 1], gz = m[3 * a + 2];
+            const double inv = 1.0 / sqrt(gx * gx + gy * gy + gz * gz);
+            const double sgn = (f & 1) ? inv : -inv;
+            const double nx = sgn * gx, ny = sgn * gy, nz = sgn * gz;
+            const double rn = ru * nx + rv * ny + rw * nz;
+            ru -= rn * nx; rv -= rn * ny; rw -= rn * nz;
+        }
+    }
+}
+#endif  // __CUDACC__

@@ -146,28 +146,6 @@ __device__ __forceinline__ void load_D_rows(const LglTables &t, int i, int j, in
     }
 }
 
-// No-flux wall projection at one node (A9): faces in order 0..5; n = -+ grad xi_a/|grad xi_a|.
-template <int Nq>
-__device__ __forceinline__ void wall_project(const uint8_t *__restrict__ bc, int i, int j, int k,
-                                             const double (&m)[9], double &ru, double &rv,
-                                             double &rw)
-{
-    const int idx[3] = {i, j, k};
-#pragma unroll
-    for (int f = 0; f < 6; ++f) {
-        const int a = f >> 1;
-        const bool on = bc[f] && (idx[a] == ((f & 1) ? (Nq - 1) : 0));
-        if (on) {
-            const double gx = m[3 * a + 0], gy = m[3 * a + 1], gz = m[3 * a + 2];
-            const double inv = 1.0 / sqrt(gx * gx + gy * gy + gz * gz);
-            const double sgn = (f & 1) ? inv : -inv;
-            const double nx = sgn * gx, ny = sgn * gy, nz = sgn * gz;
-            const double rn = ru * nx + rv * ny + rw * nz;
-            ru -= rn * nx; rv -= rn * ny; rw -= rn * nz;
-        }
-    }
-}
-
 // ---------------------------------------------------------------------------------------
 // numa_rhs: rhs = omega * S(q)   (A2-A6)
 // ---------------------------------------------------------------------------------------
@@ -206,25 +184,6 @@ k_rhs(const double *__restrict__ q, const double *__restrict__ ref3,
     const double om = omega[p];
 #pragma unroll
     for (int c = 0; c < 5; ++c) rhs[c * NL + p] = om * S[c];
-}
-
-// ---------------------------------------------------------------------------------------
-// numa_dss_or_flux (CG): deterministic DSS, one thread per SHARED global node
-// ---------------------------------------------------------------------------------------
-__global__ void k_dss(double *__restrict__ r, const int32_t *__restrict__ sh_nodes,
-                      const int32_t *__restrict__ start, const int32_t *__restrict__ copies,
-                      int64_t n_shared, int64_t NL, int nf)
-{
-    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= n_shared) return;
-    const int gI = sh_nodes[t];
-    const int s = start[gI], c = start[gI + 1] - s;
-    for (int m = 0; m < nf; ++m) {
-        double *rm = r + (int64_t)m * NL;
-        double sum = 0.0;
-        for (int a = 0; a < c; ++a) sum += rm[copies[s + a]];
-        for (int a = 0; a < c; ++a) rm[copies[s + a]] = sum;
-    }
 }
 
 // mass: M = sum over copies of wJ (all global nodes), omega = wJ / M, in place on `om`
@@ -393,16 +352,6 @@ cudaError_t launch_rhs(numa_ctx *c, const double *q, double *rhs, cudaStream_t s
 {
     LaunchScope ls(c, K_VOLUME, s);
     DISPATCH_N(rhs_N, c, q, rhs, s);
-}
-
-cudaError_t launch_dss(numa_ctx *c, double *r, int nfields, cudaStream_t s)
-{
-    if (c->n_shared == 0) return cudaSuccess;
-    LaunchScope ls(c, K_DSS, s);
-    const int64_t blocks = (c->n_shared + 255) / 256;
-    k_dss<<<(unsigned)blocks, 256, 0, s>>>(r, c->sh_nodes, c->dss_start, c->dss_copies,
-                                           c->n_shared, c->NL, nfields);
-    return cudaGetLastError();
 }
 
 cudaError_t launch_mass(numa_ctx *c, cudaStream_t s)
