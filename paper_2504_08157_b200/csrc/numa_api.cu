@@ -116,7 +116,7 @@ static WsLayout ws_layout(const numa_params *p)
     L.sh_nodes = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
     L.dss_idx = off; off = align_up(off + NL * 4);
     L.face_bc = off; off = align_up(off + (size_t)p->n_elem * 8);
-    L.flags = off; off = align_up(off + 64);
+    L.flags = off; off = align_up(off + 256);
     L.small_tmp = off; off = align_up(off + kSmallTmp);
     L.total = off;
     return L;
@@ -305,7 +305,7 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
         void *cub_tmp = (void *)align_up((size_t)(valsB + NL));
         size_t cub_avail = (char *)cub_tmp < ws + L.omega ? (size_t)((ws + L.omega) - (char *)cub_tmp) : 0;
         if (cub_avail < kSmallTmp) { cub_tmp = ws + L.small_tmp; cub_avail = kSmallTmp; }
-        CK(cudaMemsetAsync(c->d_flags, 0, 64, s));
+        CK(cudaMemsetAsync(c->d_flags, 0, 256, s));
         k_iota_check<<<grid_for(NL), 256, 0, s>>>(valsA, intma_cg, keysA, NL, NG, c->d_flags);
         CK(cudaGetLastError());
         c->launches++;
@@ -326,7 +326,7 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
             SharedPred pred{c->dss_start};
             thrust::counting_iterator<int32_t> ids(0);
             int32_t *d_num = c->d_flags + 8;
-            unsigned long long *d_cnt = (unsigned long long *)(c->d_flags + 10);  // 4 counters
+            unsigned long long *d_cnt = (unsigned long long *)(c->d_flags + 16);  // 4 counters
             char *scr2 = (char *)align_up((size_t)(valsB + NL));
             char *scr_end = ws + L.omega;
             int32_t *nodesA = (int32_t *)scr2;                         // [NG]

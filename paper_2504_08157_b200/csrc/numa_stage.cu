@@ -14,25 +14,38 @@
 namespace {
 
 // ---------------------------------------------------------------------------------------
-// Column-marching layout: thread (le, i, j) owns the zeta-column k = 0..N of element le of the
-// block.  zeta-derivatives are taken in registers with D as compile-time-indexed constant-bank
-// operands; xi- and eta-derivatives are taken by the same threads re-indexed as line owners
-// (one whole line of the contraction per thread, again with constant-bank D), exchanging
-// through shared memory: 1 store + 2x(1 load + 1 store) + 2 loads per field and node instead
-// of the 3(N+1) loads of a thread-per-node contraction.
-// Shared-memory node index: i + SJ*j + SK*k with SJ odd (bank-conflict-free line access).
+// Volume kernel layout.  A block owns EPB consecutive elements (a contiguous chunk of
+// EPB*Mn nodes of every field).  Pointwise work (A2 pre-pass; A5-A10 combine) is done one
+// thread per node, so every global access is coalesced.  The 24 one-dimensional contractions
+// of Alg. 2 are done as LINE TASKS: one thread takes one whole line of one field along one
+// direction (N+1 shared loads), forms all N+1 derivatives of the line with D as
+// compile-time-indexed constant-bank operands ((N+1)^2 FMAs, no further loads) and stores
+// them (N+1 shared stores).  Per node and field that is 1 store + 3x(1 load + 1 store) + 3
+// loads of shared memory instead of the 3(N+1) loads of a thread-per-node contraction.
+// The zeta-derivatives overwrite the work fields in place (after a barrier), so a node needs
+// 24 doubles of shared memory.  Shared node index: i + SJ*j + SK*k, SJ odd (bank-conflict-
+// free xi-lines).
 // ---------------------------------------------------------------------------------------
-template <int N, int EPB_>
+template <int N>
 struct StageShape {
     static constexpr int Nq = N + 1, N2 = Nq * Nq, Mn = N2 * Nq;
-    static constexpr int EPB = EPB_;
+#ifndef STAGE_EPB4
+#define STAGE_EPB4 2
+#endif
+#ifndef STAGE_MINB4
+#define STAGE_MINB4 3
+#endif
+    static constexpr int EPB = (N == 2) ? 9 : (N == 3) ? 4 : (N == 4) ? STAGE_EPB4 : 1;
     static constexpr int SJ = (Nq & 1) ? Nq : Nq + 1;
     static constexpr int SK = SJ * Nq;
     static constexpr int ME = SK * Nq;  // padded nodes per element and field
     static constexpr int NF = 8;        // p', u, v, w, theta, Fx, Fy, Fz
-    static constexpr int ACTIVE = EPB * N2;
-    static constexpr int THREADS = (ACTIVE + 31) / 32 * 32;
-    static constexpr size_t SMEM = sizeof(double) * 3 * NF * EPB * ME;
+    static constexpr int NODES = EPB * Mn;
+    static constexpr int THREADS = (NODES + 31) / 32 * 32;
+    static constexpr int LINES = EPB * N2;  // lines per field and direction
+    static constexpr int FS = EPB * ME;     // field stride in shared memory
+    static constexpr size_t SMEM = sizeof(double) * 3 * NF * FS;
+    static constexpr int MIN_BLOCKS = (N == 4) ? STAGE_MINB4 : (N < 4) ? 3 : (N <= 6) ? 2 : 1;
 };
 
 struct StageArgs {
@@ -42,170 +55,182 @@ struct StageArgs {
     const uint8_t *face_bc;
     int64_t Ne, NL;
     double g, gamma, f_cor, a0, a1, b_dt;
+    double eos[14];  // binomial(gamma, n), n = 1..14: (1+x)^gamma - 1 = sum_n eos[n-1] x^n
     int has_walls;
 };
 
-template <int N, int EPB>
-__global__ void __launch_bounds__(StageShape<N, EPB>::THREADS)
+// Eq. 3 in cancellation-free form (Q6): p'/p0 = (1+x)^gamma - 1 with
+// 1 + x = (1 + rho'/rho0)(1 + theta'/theta0).  For |x| <= 1/16 the binomial series to degree
+// 14 is exact to double rounding (next term < 2e-20 |x|); otherwise expm1(gamma log1p(x)).
+__device__ __forceinline__ double eos_ratio(double x, double gamma, const double (&c)[14])
+{
+    if (fabs(x) <= 0.0625) {
+        double s = c[13];
+#pragma unroll
+        for (int n = 12; n >= 0; --n) s = fma(s, x, c[n]);
+        return s * x;
+    }
+    return expm1(gamma * log1p(x));
+}
+
+template <int Nq>
+__device__ __forceinline__ void line_derivs(const double *src, int sstride, double *dst,
+                                            const LglTables &tab)
+{
+    double x[Nq];
+#pragma unroll
+    for (int l = 0; l < Nq; ++l) x[l] = src[sstride * l];
+#pragma unroll
+    for (int m = 0; m < Nq; ++m) {
+        double acc = 0.0;
+#pragma unroll
+        for (int l = 0; l < Nq; ++l) acc = fma(tab.D[m * Nq + l], x[l], acc);
+        dst[sstride * m] = acc;
+    }
+}
+
+template <int N>
+__global__ void __launch_bounds__(StageShape<N>::THREADS, StageShape<N>::MIN_BLOCKS)
 k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglTables tab)
 {
-    using SH = StageShape<N, EPB>;
+    using SH = StageShape<N>;
     constexpr int Nq = SH::Nq, N2 = SH::N2, Mn = SH::Mn, SJ = SH::SJ, SK = SH::SK, ME = SH::ME,
-                  NF = SH::NF;
+                  NF = SH::NF, FS = SH::FS, LINES = SH::LINES;
     extern __shared__ double smem[];
-    double *sW = smem;                    // [NF][EPB][ME] nodal work fields
-    double *sGx = sW + NF * EPB * ME;     // d/dxi
-    double *sGe = sGx + NF * EPB * ME;    // d/deta
+    double *sW = smem;            // [NF][EPB][ME] nodal work fields, later d/dzeta
+    double *sGx = sW + NF * FS;   // d/dxi
+    double *sGe = sGx + NF * FS;  // d/deta
 
     const int tid = threadIdx.x;
-    const int le = tid / N2, ij = tid - le * N2;
-    const int j = ij / Nq, i = ij - j * Nq;
-    const int64_t e = (int64_t)blockIdx.x * EPB + le;
-    const bool active = (tid < SH::ACTIVE) && (e < A.Ne);
     const int64_t NL = A.NL;
-    const int64_t pb = e * Mn + ij;            // global index of node (i, j, 0)
-    const int sb = le * ME + i + SJ * j;       // shared index of node (i, j, 0)
+    const int64_t node0 = (int64_t)blockIdx.x * SH::NODES;
+    const int64_t rem = NL - node0;
+    const int n_nodes = rem < SH::NODES ? (int)rem : SH::NODES;  // ragged last block
+    const int n_lines = n_nodes / Nq;                            // = elements * N2
 
-    // ---- phase A: pointwise pre-pass (A2) down the column, zeta-derivatives in registers ----
-    double Gz[NF][Nq];
-    if (active) {
-        const double *__restrict__ r0 = A.ref3, *__restrict__ r1 = A.ref3 + NL,
-                                   *__restrict__ r2 = A.ref3 + 2 * NL;
-        const double th0e = r1[e * Mn];  // theta0 relative to the element's first node (Q7)
-        double W[NF][Nq];
-#pragma unroll
-        for (int k = 0; k < Nq; ++k) {
-            const int64_t p = pb + (int64_t)k * N2;
-            const double rhop = A.qs[p], u = A.qs[NL + p], v = A.qs[2 * NL + p],
-                         w = A.qs[3 * NL + p], thp = A.qs[4 * NL + p];
-            const double rho0 = r0[p], th0 = r1[p], p0 = r2[p];
-            // Eq. 3, cancellation-free: p' = p0 expm1(gamma log1p(x)), 1+x = (1+a)(1+b)  (Q6)
-            const double a = rhop / rho0, b = thp / th0;
-            const double x = a + b + a * b;
-            const double rho = rho0 + rhop;
-            W[0][k] = p0 * expm1(A.gamma * log1p(x));
-            W[1][k] = u;
-            W[2][k] = v;
-            W[3][k] = w;
-            W[4][k] = thp + (th0 - th0e);
-            W[5][k] = rho * u;
-            W[6][k] = rho * v;
-            W[7][k] = rho * w;
-#pragma unroll
-            for (int f = 0; f < NF; ++f) sW[f * EPB * ME + sb + SK * k] = W[f][k];
-        }
-#pragma unroll
-        for (int f = 0; f < NF; ++f)
-#pragma unroll
-            for (int k = 0; k < Nq; ++k) {
-                double acc = 0.0;
-#pragma unroll
-                for (int l = 0; l < Nq; ++l) acc = fma(tab.D[k * Nq + l], W[f][l], acc);
-                Gz[f][k] = acc;
-            }
-    }
-    __syncthreads();
+    // this thread's node (pointwise role)
+    const bool has_node = tid < n_nodes;
+    const int le = tid / Mn, n = tid - le * Mn;
+    const int k = n / N2, j = (n - k * N2) / Nq, i = n - k * N2 - j * Nq;
+    const int sp = le * ME + i + SJ * j + SK * k;
+    const int64_t p = node0 + tid;
 
-    // ---- phase B: xi- and eta-lines (Alg. 2), one whole line per thread and field ----------
-    if (active) {
-        // this thread's xi-line: (le, j' = i_line, k' = j_line) -> nodes l + SJ*(jk)
-        const int xb = le * ME + SJ * ij;                      // line index jk = ij
-        // this thread's eta-line: (le, i' = i, k' = j)  -> nodes i + SJ*l + SK*j
-        const int eb = le * ME + i + SK * j;
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            const double *w = sW + f * EPB * ME;
-            double x[Nq], y[Nq];
-#pragma unroll
-            for (int l = 0; l < Nq; ++l) { x[l] = w[xb + l]; y[l] = w[eb + SJ * l]; }
-            double *gx = sGx + f * EPB * ME, *ge = sGe + f * EPB * ME;
-#pragma unroll
-            for (int m = 0; m < Nq; ++m) {
-                double ax = 0.0, ay = 0.0;
-#pragma unroll
-                for (int l = 0; l < Nq; ++l) {
-                    ax = fma(tab.D[m * Nq + l], x[l], ax);
-                    ay = fma(tab.D[m * Nq + l], y[l], ay);
-                }
-                gx[xb + m] = ax;
-                ge[eb + SJ * m] = ay;
-            }
-        }
-    }
-    __syncthreads();
-    if (!active) return;
-
-    // ---- phase C: chain rule, Eq. 1 tendencies, sources, walls, stage update (A5-A10) -------
-    const uint2 bcw = *reinterpret_cast<const uint2 *>(A.face_bc + e * 8);
-    uint8_t bc[8];
-#pragma unroll
-    for (int f = 0; f < 4; ++f) {
-        bc[f] = (uint8_t)(bcw.x >> (8 * f));
-        bc[4 + f] = (uint8_t)(bcw.y >> (8 * f));
-    }
-    const bool elem_walls = A.has_walls && ((bcw.x | bcw.y) != 0);
-    const bool same = (A.q0 == A.qs);
-#pragma unroll
-    for (int k = 0; k < Nq; ++k) {
-        const int64_t p = pb + (int64_t)k * N2;
-        const int sp = sb + SK * k;
-        double m[9];
-#pragma unroll
-        for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
-        const double om = __ldg(A.omega + p);
-        const double rho0 = __ldg(A.ref3 + p);
-        double qv[5], q0v[5];
+    // ---- phase A: pointwise pre-pass (A2) ---------------------------------------------------
+    double qv[5] = {0, 0, 0, 0, 0}, rho0 = 1.0;
+    if (has_node) {
 #pragma unroll
         for (int c = 0; c < 5; ++c) qv[c] = A.qs[c * NL + p];
-        if (same) {
-#pragma unroll
-            for (int c = 0; c < 5; ++c) q0v[c] = qv[c];
-        } else {
-#pragma unroll
-            for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
-        }
-        double fx[NF], fe[NF];
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-            fx[f] = sGx[f * EPB * ME + sp];
-            fe[f] = sGe[f * EPB * ME + sp];
-        }
-        const double rhop = qv[0], u = qv[1], v = qv[2], w = qv[3];
-        const double irho = 1.0 / (rho0 + rhop);
-        // contravariant velocity: u . grad f = sum_a U^a f_{xi_a}
-        const double Ux = u * m[0] + v * m[1] + w * m[2];
-        const double Ue = u * m[3] + v * m[4] + w * m[5];
-        const double Uz = u * m[6] + v * m[7] + w * m[8];
-        const double px = fx[0] * m[0] + fe[0] * m[3] + Gz[0][k] * m[6];
-        const double py = fx[0] * m[1] + fe[0] * m[4] + Gz[0][k] * m[7];
-        const double pz = fx[0] * m[2] + fe[0] * m[5] + Gz[0][k] * m[8];
-        double S[5];
-        S[1] = -(Ux * fx[1] + Ue * fe[1] + Uz * Gz[1][k]) - px * irho;
-        S[2] = -(Ux * fx[2] + Ue * fe[2] + Uz * Gz[2][k]) - py * irho;
-        S[3] = -(Ux * fx[3] + Ue * fe[3] + Uz * Gz[3][k]) - pz * irho - (rhop * irho) * A.g;
-        S[4] = -(Ux * fx[4] + Ue * fe[4] + Uz * Gz[4][k]);
-        double div = fx[5] * m[0] + fe[5] * m[3] + Gz[5][k] * m[6];
-        div += fx[6] * m[1] + fe[6] * m[4] + Gz[6][k] * m[7];
-        div += fx[7] * m[2] + fe[7] * m[5] + Gz[7][k] * m[8];
-        S[0] = -div;
-        // A8: heating, Coriolis, sponge
-        if (A.heat) S[4] += __ldg(A.heat + p);
-        S[1] += A.f_cor * v;
-        S[2] -= A.f_cor * u;
-        if (A.beta) {
-            const double b = __ldg(A.beta + p);
-            S[1] -= b * u; S[2] -= b * v; S[3] -= b * w; S[4] -= b * qv[4];
-        }
-        // A6: weight; A9: walls on the weighted velocity tendency
-        double r[5];
-#pragma unroll
-        for (int c = 0; c < 5; ++c) r[c] = om * S[c];
-        if (elem_walls) wall_project<Nq>(bc, i, j, k, m, r[1], r[2], r[3]);
-        // A10 as a DSS partial sum
-#pragma unroll
-        for (int c = 0; c < 5; ++c)
-            A.qout[c * NL + p] = om * (A.a0 * q0v[c] + A.a1 * qv[c]) + A.b_dt * r[c];
+        rho0 = __ldg(A.ref3 + p);
+        const double th0 = __ldg(A.ref3 + NL + p), p0 = __ldg(A.ref3 + 2 * NL + p);
+        const double th0e = __ldg(A.ref3 + NL + (p - n));  // theta0 at the element's first node (Q7)
+        const double x = (qv[0] * th0 + qv[4] * rho0 + qv[0] * qv[4]) / (rho0 * th0);
+        const double rho = rho0 + qv[0];
+        sW[0 * FS + sp] = p0 * eos_ratio(x, A.gamma, A.eos);
+        sW[1 * FS + sp] = qv[1];
+        sW[2 * FS + sp] = qv[2];
+        sW[3 * FS + sp] = qv[3];
+        sW[4 * FS + sp] = qv[4] + (th0 - th0e);
+        sW[5 * FS + sp] = rho * qv[1];
+        sW[6 * FS + sp] = rho * qv[2];
+        sW[7 * FS + sp] = rho * qv[3];
     }
+    __syncthreads();
+
+    // ---- phase B: line tasks (Alg. 2): xi and eta (both only read sW), then zeta in place ----
+    for (int t = tid; t < NF * LINES; t += SH::THREADS) {
+        const int f = t / LINES, line = t - f * LINES;
+        if (line >= n_lines) continue;
+        const int el = line / N2, l2 = line - el * N2;
+        const int a = l2 / Nq, b = l2 - a * Nq;  // l2 = b + Nq*a
+        const int base = f * FS + el * ME;
+        // xi-line (j, k) = (b, a): nodes l + SJ*l2
+        line_derivs<Nq>(sW + base + SJ * l2, 1, sGx + base + SJ * l2, tab);
+        // eta-line (i, k) = (b, a): nodes b + SJ*l + SK*a
+        line_derivs<Nq>(sW + base + b + SK * a, SJ, sGe + base + b + SK * a, tab);
+    }
+    __syncthreads();
+    for (int t = tid; t < NF * LINES; t += SH::THREADS) {
+        const int f = t / LINES, line = t - f * LINES;
+        if (line >= n_lines) continue;
+        const int el = line / N2, l2 = line - el * N2;
+        const int a = l2 / Nq, b = l2 - a * Nq;
+        // zeta-line (i, j) = (b, a): nodes b + SJ*a + SK*l, derivative written in place
+        double *w = sW + f * FS + el * ME + b + SJ * a;
+        line_derivs<Nq>(w, SK, w, tab);
+    }
+    __syncthreads();
+    if (!has_node) return;
+
+    // ---- phase C: chain rule, Eq. 1 tendencies, sources, walls, stage update (A5-A10) -------
+    double m[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
+    const double om = __ldg(A.omega + p);
+    double q0v[5];
+    if (A.q0 == A.qs) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) q0v[c] = qv[c];
+    } else {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+    }
+    double fx[NF], fe[NF], fz[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+        fx[f] = sGx[f * FS + sp];
+        fe[f] = sGe[f * FS + sp];
+        fz[f] = sW[f * FS + sp];
+    }
+    const double rhop = qv[0], u = qv[1], v = qv[2], w = qv[3];
+    const double irho = 1.0 / (rho0 + rhop);
+    // contravariant velocity: u . grad f = sum_a U^a f_{xi_a}
+    const double Ux = u * m[0] + v * m[1] + w * m[2];
+    const double Ue = u * m[3] + v * m[4] + w * m[5];
+    const double Uz = u * m[6] + v * m[7] + w * m[8];
+    const double px = fx[0] * m[0] + fe[0] * m[3] + fz[0] * m[6];
+    const double py = fx[0] * m[1] + fe[0] * m[4] + fz[0] * m[7];
+    const double pz = fx[0] * m[2] + fe[0] * m[5] + fz[0] * m[8];
+    double S[5];
+    S[1] = -(Ux * fx[1] + Ue * fe[1] + Uz * fz[1]) - px * irho;
+    S[2] = -(Ux * fx[2] + Ue * fe[2] + Uz * fz[2]) - py * irho;
+    S[3] = -(Ux * fx[3] + Ue * fe[3] + Uz * fz[3]) - pz * irho - (rhop * irho) * A.g;
+    S[4] = -(Ux * fx[4] + Ue * fe[4] + Uz * fz[4]);
+    double div = fx[5] * m[0] + fe[5] * m[3] + fz[5] * m[6];
+    div += fx[6] * m[1] + fe[6] * m[4] + fz[6] * m[7];
+    div += fx[7] * m[2] + fe[7] * m[5] + fz[7] * m[8];
+    S[0] = -div;
+    // A8: heating, Coriolis, sponge
+    if (A.heat) S[4] += __ldg(A.heat + p);
+    S[1] += A.f_cor * v;
+    S[2] -= A.f_cor * u;
+    if (A.beta) {
+        const double b = __ldg(A.beta + p);
+        S[1] -= b * u; S[2] -= b * v; S[3] -= b * w; S[4] -= b * qv[4];
+    }
+    // A6: weight; A9: walls on the weighted velocity tendency
+    double r[5];
+#pragma unroll
+    for (int c = 0; c < 5; ++c) r[c] = om * S[c];
+    if (A.has_walls) {
+        const bool on_face = (i == 0) | (i == Nq - 1) | (j == 0) | (j == Nq - 1) | (k == 0) | (k == Nq - 1);
+        if (on_face) {
+            const int64_t e = (p - n) / Mn;
+            const uint2 bcw = *reinterpret_cast<const uint2 *>(A.face_bc + e * 8);
+            if (bcw.x | bcw.y) {
+                uint8_t bc[8];
+#pragma unroll
+                for (int f = 0; f < 4; ++f) {
+                    bc[f] = (uint8_t)(bcw.x >> (8 * f));
+                    bc[4 + f] = (uint8_t)(bcw.y >> (8 * f));
+                }
+                wall_project<Nq>(bc, i, j, k, m, r[1], r[2], r[3]);
+            }
+        }
+    }
+    // A10 as a DSS partial sum
+#pragma unroll
+    for (int c = 0; c < 5; ++c)
+        A.qout[c * NL + p] = om * (A.a0 * q0v[c] + A.a1 * qv[c]) + A.b_dt * r[c];
 }
 
 // ---------------------------------------------------------------------------------------
@@ -275,19 +300,19 @@ k_stage_dss(double *r, const __grid_constant__ DssArgs A)
     }
 }
 
-template <int N, int EPB>
+template <int N>
 cudaError_t stage_launch(numa_ctx *c, const StageArgs &a, cudaStream_t s)
 {
-    using SH = StageShape<N, EPB>;
+    using SH = StageShape<N>;
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_stage_volume<N, EPB>,
+        cudaError_t e = cudaFuncSetAttribute(k_stage_volume<N>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SH::SMEM);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int64_t blocks = (c->par.n_elem + EPB - 1) / EPB;
-    k_stage_volume<N, EPB><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a, c->lgl);
+    const int64_t blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
+    k_stage_volume<N><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a, c->lgl);
     return cudaGetLastError();
 }
 
@@ -305,14 +330,22 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
     a.g = c->par.g; a.gamma = c->gamma; a.f_cor = c->par.f_cor;
     a.a0 = a0; a.a1 = a1; a.b_dt = b_dt;
     a.has_walls = c->has_walls;
+    // binomial(gamma, n): c_1 = gamma, c_{n+1} = c_n (gamma - n) / (n + 1)
+    {
+        long double cn = (long double)c->gamma;
+        for (int n = 1; n <= 14; ++n) {
+            a.eos[n - 1] = (double)cn;
+            cn = cn * ((long double)c->gamma - n) / (n + 1);
+        }
+    }
     switch (c->par.N) {
-        case 2: return stage_launch<2, 8>(c, a, s);
-        case 3: return stage_launch<3, 4>(c, a, s);
-        case 4: return stage_launch<4, 4>(c, a, s);
-        case 5: return stage_launch<5, 2>(c, a, s);
-        case 6: return stage_launch<6, 1>(c, a, s);
-        case 7: return stage_launch<7, 1>(c, a, s);
-        case 8: return stage_launch<8, 1>(c, a, s);
+        case 2: return stage_launch<2>(c, a, s);
+        case 3: return stage_launch<3>(c, a, s);
+        case 4: return stage_launch<4>(c, a, s);
+        case 5: return stage_launch<5>(c, a, s);
+        case 6: return stage_launch<6>(c, a, s);
+        case 7: return stage_launch<7>(c, a, s);
+        case 8: return stage_launch<8>(c, a, s);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -205,7 +205,12 @@ def test_100_rk3_steps_parity(cfg, N, scale, steps):
         g.rk_stage(s1[0], s1[1], s1[2] * dt, qb, qb, g.full_rhs(qb, hd0), q1)
         g.rk_stage(s2[0], s2[1], s2[2] * dt, qb, q1, g.full_rhs(q1, hd0), q1)
         g.rk_stage(s3[0], s3[1], s3[2] * dt, qb, q1, g.full_rhs(q1, hd0), qb)
-    e2 = rel_l2(_np(qa), _np(qb))
+    # (velocity components that are small by symmetry carry the rounding of the large one:
+    # they are scaled by the norm of the whole velocity)
+    a, b = _np(qa), _np(qb)
+    vel = np.sqrt(sum(np.linalg.norm(b[m]) ** 2 for m in (1, 2, 3)))
+    den = [np.linalg.norm(b[0]), vel, vel, vel, np.linalg.norm(b[4])]
+    e2 = np.array([np.linalg.norm(a[m] - b[m]) / (den[m] if den[m] > 0 else 1.0) for m in range(5)])
     assert np.all(e2 <= 1e-13), e2
 
 
