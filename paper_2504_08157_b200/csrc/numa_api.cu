@@ -91,9 +91,11 @@ static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a
 static const size_t kSmallTmp = (size_t)4 << 20;  // CUB temp storage for small meshes
 
 struct WsLayout {
-    size_t met, omega, ref3, sponge, start, copies, sh_nodes, dss_idx, face_bc, flags, small_tmp, total;
+    size_t met, omega, ref3, sponge, start, copies, sh_nodes, dss_idx, dss_seg, dss_blkmap, face_bc, flags, small_tmp, total;
     size_t scratch_bytes;  // init-time scratch, aliased onto the (not yet written) met region
 };
+
+static inline size_t WsMaxSeg(size_t NL) { return 4 * (NL / NUMA_DSS_CHUNK + 2); }
 
 static bool params_ok(const numa_params *p)
 {
@@ -115,6 +117,9 @@ static WsLayout ws_layout(const numa_params *p)
     L.copies = off; off = align_up(off + NL * 4);
     L.sh_nodes = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
     L.dss_idx = off; off = align_up(off + NL * 4);
+    const size_t max_seg = WsMaxSeg(NL);
+    L.dss_seg = off; off = align_up(off + max_seg * sizeof(DssSeg));
+    L.dss_blkmap = off; off = align_up(off + ((size_t)p->n_global / NUMA_DSS_THREADS + max_seg + 1) * 4);
     L.face_bc = off; off = align_up(off + (size_t)p->n_elem * 8);
     L.flags = off; off = align_up(off + 256);
     L.small_tmp = off; off = align_up(off + kSmallTmp);
@@ -169,32 +174,46 @@ struct SharedPred {
     __device__ bool operator()(int32_t g) const { return start[g + 1] - start[g] >= 2; }
 };
 
-// sort key of a shared node: (multiplicity class, first copy); class 0,1,2 = 2,4,8 copies,
-// 3 = anything else.  Counts the classes in cnt[0..3].
+// sort key of a shared node: (chunk of its first copy, multiplicity class, first copy);
+// class 0,1,2 = 2,4,8 copies, 3 = anything else.
 __global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *__restrict__ start,
                              const int32_t *__restrict__ copies, uint64_t *__restrict__ keys,
-                             int64_t n, unsigned long long *cnt)
+                             int64_t n)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
         const int32_t g = nodes[t];
         const int32_t s = start[g], c = start[g + 1] - s;
         const uint64_t cls = (c == 2) ? 0 : (c == 4) ? 1 : (c == 8) ? 2 : 3;
-        keys[t] = (cls << 32) | (uint32_t)copies[s];
-        atomicAdd(cnt + cls, 1ULL);
+        const uint32_t first = (uint32_t)copies[s];
+        keys[t] = ((uint64_t)(first / NUMA_DSS_CHUNK) << 34) | (cls << 32) | first;
     }
 }
 
-// transposed copy lists of one class: idx[a*n + t] = a-th copy of the t-th node
-__global__ void k_class_lists(const int32_t *__restrict__ nodes, const int32_t *__restrict__ start,
-                              const int32_t *__restrict__ copies, int32_t *__restrict__ idx,
-                              int64_t n, int C)
+struct SegHeadPred {
+    const uint64_t *keys;
+    __device__ bool operator()(int32_t t) const { return t == 0 || (keys[t] >> 32) != (keys[t - 1] >> 32); }
+};
+
+__global__ void k_gather_hi(const uint64_t *__restrict__ keys, const int32_t *__restrict__ heads,
+                            int32_t *__restrict__ hi, int n)
 {
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
-        const int32_t s = start[nodes[t]];
-        for (int a = 0; a < C; ++a) idx[(int64_t)a * n + t] = copies[s + a];
-    }
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) hi[t] = (int32_t)(keys[heads[t]] >> 32);
+}
+
+// transposed copy lists: one thread per shared node, indexed exactly like the DSS kernel
+__global__ void __launch_bounds__(NUMA_DSS_THREADS)
+k_class_lists(const int32_t *__restrict__ nodes, const int32_t *__restrict__ start,
+              const int32_t *__restrict__ copies, int32_t *__restrict__ idx,
+              const DssSeg *__restrict__ segs, const int32_t *__restrict__ blkmap)
+{
+    const DssSeg sg = segs[blkmap[blockIdx.x]];
+    const int t = (blockIdx.x - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
+    if (t >= sg.n || sg.cls > 2) return;
+    const int C = 2 << sg.cls;
+    const int32_t s = start[nodes[sg.node_off + t]];
+    for (int a = 0; a < C; ++a) idx[sg.idx_base + (int64_t)a * sg.n + t] = copies[s + a];
 }
 
 __global__ void k_ref3(const double *__restrict__ ref, double *__restrict__ ref3, int64_t NL,
@@ -291,6 +310,8 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
     c->dss_copies = (int32_t *)(ws + L.copies);
     c->sh_nodes = (int32_t *)(ws + L.sh_nodes);
     c->dss_idx = (int32_t *)(ws + L.dss_idx);
+    c->dss_seg = (DssSeg *)(ws + L.dss_seg);
+    c->dss_blkmap = (int32_t *)(ws + L.dss_blkmap);
     c->face_bc = (uint8_t *)(ws + L.face_bc);
     c->d_flags = (int32_t *)(ws + L.flags);
     {
@@ -326,7 +347,6 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
             SharedPred pred{c->dss_start};
             thrust::counting_iterator<int32_t> ids(0);
             int32_t *d_num = c->d_flags + 8;
-            unsigned long long *d_cnt = (unsigned long long *)(c->d_flags + 16);  // 4 counters
             char *scr2 = (char *)align_up((size_t)(valsB + NL));
             char *scr_end = ws + L.omega;
             int32_t *nodesA = (int32_t *)scr2;                         // [NG]
@@ -344,38 +364,63 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
             CK(cudaMemcpyAsync(&h_num, d_num, 4, cudaMemcpyDeviceToHost, s));
             CK(cudaStreamSynchronize(s));
             c->n_shared = h_num;
-            for (int k = 0; k < 3; ++k) { c->cls_n[k] = 0; c->cls_base[k] = 0; }
-            c->n_gen = 0;
-            c->gen_nodes = c->sh_nodes;
+            c->n_seg = 0;
+            c->dss_blocks = 0;
             if (h_num > 0) {
-                k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, c->dss_start, c->dss_copies, kA,
-                                                            h_num, d_cnt);
+                k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, c->dss_start, c->dss_copies, kA, h_num);
                 CK(cudaGetLastError());
+                int end_bit2 = 35;
+                while (((int64_t)NUMA_DSS_CHUNK << (end_bit2 - 34)) < NL) ++end_bit2;
                 cub::DoubleBuffer<uint64_t> dk2(kA, kB);
                 cub::DoubleBuffer<int32_t> dv2(nodesA, nodesB);
-                CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, dk2, dv2, h_num, 0, 34, s));
+                CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, dk2, dv2, h_num, 0, end_bit2, s));
                 if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
-                CK(cub::DeviceRadixSort::SortPairs(tmp2, need2, dk2, dv2, h_num, 0, 34, s));
+                CK(cub::DeviceRadixSort::SortPairs(tmp2, need2, dk2, dv2, h_num, 0, end_bit2, s));
                 CK(cudaMemcpyAsync(c->sh_nodes, dv2.Current(), (size_t)h_num * 4, cudaMemcpyDeviceToDevice, s));
-                unsigned long long h_cnt[4] = {0, 0, 0, 0};
-                CK(cudaMemcpyAsync(h_cnt, d_cnt, 32, cudaMemcpyDeviceToHost, s));
+                // segment heads (positions where (chunk, class) changes), ascending
+                int32_t *heads = dv2.Alternate();           // [<= h_num], free after the sort
+                int32_t *hi = heads + WsMaxSeg(NL);
+                SegHeadPred hp{dk2.Current()};
+                CK(cub::DeviceSelect::If(nullptr, need2, ids, heads, d_num, h_num, hp, s));
+                if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
+                CK(cub::DeviceSelect::If(tmp2, need2, ids, heads, d_num, h_num, hp, s));
+                int32_t n_seg = 0;
+                CK(cudaMemcpyAsync(&n_seg, d_num, 4, cudaMemcpyDeviceToHost, s));
                 CK(cudaStreamSynchronize(s));
-                int64_t node_off = 0, idx_off = 0;
-                for (int k = 0; k < 3; ++k) {
-                    const int C = 2 << k;
-                    c->cls_n[k] = (int64_t)h_cnt[k];
-                    c->cls_base[k] = idx_off;
-                    if (c->cls_n[k] > 0) {
-                        k_class_lists<<<grid_for(c->cls_n[k]), 256, 0, s>>>(
-                            c->sh_nodes + node_off, c->dss_start, c->dss_copies, c->dss_idx + idx_off,
-                            c->cls_n[k], C);
-                        CK(cudaGetLastError());
-                    }
-                    node_off += c->cls_n[k];
-                    idx_off += c->cls_n[k] * C;
+                if ((size_t)n_seg > WsMaxSeg(NL)) { errstr = "internal: DSS segment table does not fit"; goto cuda_fail; }
+                k_gather_hi<<<(n_seg + 255) / 256, 256, 0, s>>>(dk2.Current(), heads, hi, n_seg);
+                CK(cudaGetLastError());
+                std::vector<int32_t> h_heads(n_seg), h_hi(n_seg);
+                CK(cudaMemcpyAsync(h_heads.data(), heads, (size_t)n_seg * 4, cudaMemcpyDeviceToHost, s));
+                CK(cudaMemcpyAsync(h_hi.data(), hi, (size_t)n_seg * 4, cudaMemcpyDeviceToHost, s));
+                CK(cudaStreamSynchronize(s));
+                std::vector<DssSeg> h_seg(n_seg);
+                std::vector<int32_t> h_map;
+                int64_t idx_off = 0, blk = 0;
+                for (int k = 0; k < n_seg; ++k) {
+                    DssSeg &sg = h_seg[k];
+                    sg.node_off = h_heads[k];
+                    sg.n = (k + 1 < n_seg ? h_heads[k + 1] : h_num) - h_heads[k];
+                    sg.cls = h_hi[k] & 3;
+                    sg.idx_base = idx_off;
+                    sg.blk0 = (int32_t)blk;
+                    sg.pad = 0;
+                    if (sg.cls < 3) idx_off += (int64_t)sg.n * (2 << sg.cls);
+                    const int nb = (sg.n + NUMA_DSS_THREADS - 1) / NUMA_DSS_THREADS;
+                    h_map.insert(h_map.end(), nb, k);
+                    blk += nb;
                 }
-                c->gen_nodes = c->sh_nodes + node_off;
-                c->n_gen = (int64_t)h_cnt[3];
+                if ((size_t)blk > (size_t)NG / NUMA_DSS_THREADS + WsMaxSeg(NL) + 1 || idx_off > NL) {
+                    errstr = "internal: DSS tables do not fit"; goto cuda_fail;
+                }
+                c->n_seg = n_seg;
+                c->dss_blocks = blk;
+                CK(cudaMemcpyAsync(c->dss_seg, h_seg.data(), (size_t)n_seg * sizeof(DssSeg), cudaMemcpyHostToDevice, s));
+                CK(cudaMemcpyAsync(c->dss_blkmap, h_map.data(), (size_t)blk * 4, cudaMemcpyHostToDevice, s));
+                k_class_lists<<<(unsigned)blk, NUMA_DSS_THREADS, 0, s>>>(c->sh_nodes, c->dss_start, c->dss_copies,
+                                                                        c->dss_idx, c->dss_seg, c->dss_blkmap);
+                CK(cudaGetLastError());
+                CK(cudaStreamSynchronize(s));  // h_seg / h_map are read by the copies above
                 c->launches += 6;
             }
         }

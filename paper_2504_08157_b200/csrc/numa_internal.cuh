@@ -19,6 +19,18 @@ struct LglTables {
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
 enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_COUNT = 6 };
 
+#define NUMA_DSS_CHUNK 32768   // local nodes per DSS locality chunk
+#define NUMA_DSS_THREADS 128   // shared nodes per thread block of the DSS kernel
+
+struct DssSeg {
+    int64_t node_off;  // first node of the segment in sh_nodes
+    int64_t idx_base;  // start of its transposed copy lists in dss_idx (classes 0..2)
+    int32_t n;         // nodes in the segment
+    int32_t cls;       // 0,1,2 = 2,4,8 copies; 3 = other
+    int32_t blk0;      // first thread block of the segment
+    int32_t pad;
+};
+
 struct ProfRec { int id; cudaEvent_t a, b; };
 
 struct numa_ctx {
@@ -36,13 +48,15 @@ struct numa_ctx {
     int32_t *dss_copies;  // [NL]    local indices, ascending within a node
     int32_t *sh_nodes;    // [n_shared] global ids of SHARED nodes (multiplicity >= 2), ascending
     int64_t n_shared;
-    // the same lists by multiplicity class C = 2, 4, 8, transposed: dss_idx[base + a*n + t] is
-    // copy a of the t-th node of the class (nodes ordered by their first copy); nodes of any
-    // other multiplicity >= 2 go through the CSR lists (gen_nodes)
-    int32_t *dss_idx;     // [<= NL]
-    int64_t cls_n[3], cls_base[3];
-    int32_t *gen_nodes;   // [n_gen] (tail of the sorted shared-node list)
-    int64_t n_gen;
+    // the same lists in the form the DSS kernel reads.  The shared nodes (sh_nodes) are sorted
+    // by (chunk of NUMA_DSS_CHUNK local nodes holding their first copy, multiplicity class,
+    // first copy); a SEGMENT is a run of equal (chunk, class).  Classes 0,1,2 = 2,4,8 copies
+    // keep their copy lists transposed in dss_idx (copy a of node t of the segment at
+    // idx_base + a*n + t); class 3 = any other multiplicity goes through the CSR lists.
+    int32_t *dss_idx;      // [<= NL]
+    DssSeg *dss_seg;       // [n_seg]
+    int32_t *dss_blkmap;   // [dss_blocks] segment of every thread block of the DSS kernel
+    int64_t n_seg, dss_blocks;
     uint8_t *face_bc;     // [Ne][8] (padded to 8 bytes per element)
     int32_t *d_flags;     // [4] device error flags
     int has_walls;

@@ -30,10 +30,10 @@ template <int N>
 struct StageShape {
     static constexpr int Nq = N + 1, N2 = Nq * Nq, Mn = N2 * Nq;
 #ifndef STAGE_EPB4
-#define STAGE_EPB4 2
+#define STAGE_EPB4 1
 #endif
 #ifndef STAGE_MINB4
-#define STAGE_MINB4 3
+#define STAGE_MINB4 6
 #endif
     static constexpr int EPB = (N == 2) ? 9 : (N == 3) ? 4 : (N == 4) ? STAGE_EPB4 : 1;
     static constexpr int SJ = (Nq & 1) ? Nq : Nq + 1;
@@ -44,7 +44,14 @@ struct StageShape {
     static constexpr int THREADS = (NODES + 31) / 32 * 32;
     static constexpr int LINES = EPB * N2;  // lines per field and direction
     static constexpr int FS = EPB * ME;     // field stride in shared memory
-    static constexpr size_t SMEM = sizeof(double) * 3 * NF * FS;
+    // POOLED: the zeta-derivatives get their own buffer, so the line tasks of all three
+    // directions form one pool without a barrier in between (better balance at low N);
+    // otherwise they overwrite the work fields in place after a barrier (less shared memory).
+#ifndef STAGE_POOLED_MAXN
+#define STAGE_POOLED_MAXN 3
+#endif
+    static constexpr bool POOLED = (N <= STAGE_POOLED_MAXN);
+    static constexpr size_t SMEM = sizeof(double) * (POOLED ? 4 : 3) * NF * FS;
     static constexpr int MIN_BLOCKS = (N == 4) ? STAGE_MINB4 : (N < 4) ? 3 : (N <= 6) ? 2 : 1;
 };
 
@@ -89,6 +96,21 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
     }
 }
 
+// A9 for the few nodes that lie on a wall face: kept out of line so that its square roots
+// and divisions do not weigh on the registers and code of the common path.
+template <int Nq>
+__device__ __noinline__ void wall_project_cold(uint2 bcw, int i, int j, int k, const double (&m)[9],
+                                               double &ru, double &rv, double &rw)
+{
+    uint8_t bc[8];
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+        bc[f] = (uint8_t)(bcw.x >> (8 * f));
+        bc[4 + f] = (uint8_t)(bcw.y >> (8 * f));
+    }
+    wall_project<Nq>(bc, i, j, k, m, ru, rv, rw);
+}
+
 template <int N>
 __global__ void __launch_bounds__(StageShape<N>::THREADS, StageShape<N>::MIN_BLOCKS)
 k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglTables tab)
@@ -117,9 +139,21 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 
     // ---- phase A: pointwise pre-pass (A2) ---------------------------------------------------
     double qv[5] = {0, 0, 0, 0, 0}, rho0 = 1.0;
+    // inputs of phase C, requested now so that they are in flight during phases A and B
+    double m[9], q0v[5], om = 0.0, heat = 0.0, beta = 0.0;
+    const bool same = (A.q0 == A.qs);
     if (has_node) {
 #pragma unroll
         for (int c = 0; c < 5; ++c) qv[c] = A.qs[c * NL + p];
+#pragma unroll
+        for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
+        om = __ldg(A.omega + p);
+        if (!same) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+        }
+        if (A.heat) heat = __ldg(A.heat + p);
+        if (A.beta) beta = __ldg(A.beta + p);
         rho0 = __ldg(A.ref3 + p);
         const double th0 = __ldg(A.ref3 + NL + p), p0 = __ldg(A.ref3 + 2 * NL + p);
         const double th0e = __ldg(A.ref3 + NL + (p - n));  // theta0 at the element's first node (Q7)
@@ -136,77 +170,78 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     }
     __syncthreads();
 
-    // ---- phase B: line tasks (Alg. 2): xi and eta (both only read sW), then zeta in place ----
-    for (int t = tid; t < NF * LINES; t += SH::THREADS) {
-        const int f = t / LINES, line = t - f * LINES;
-        if (line >= n_lines) continue;
-        const int el = line / N2, l2 = line - el * N2;
-        const int a = l2 / Nq, b = l2 - a * Nq;  // l2 = b + Nq*a
-        const int base = f * FS + el * ME;
-        // xi-line (j, k) = (b, a): nodes l + SJ*l2
-        line_derivs<Nq>(sW + base + SJ * l2, 1, sGx + base + SJ * l2, tab);
-        // eta-line (i, k) = (b, a): nodes b + SJ*l + SK*a
-        line_derivs<Nq>(sW + base + b + SK * a, SJ, sGe + base + b + SK * a, tab);
-    }
-    __syncthreads();
-    for (int t = tid; t < NF * LINES; t += SH::THREADS) {
-        const int f = t / LINES, line = t - f * LINES;
-        if (line >= n_lines) continue;
-        const int el = line / N2, l2 = line - el * N2;
-        const int a = l2 / Nq, b = l2 - a * Nq;
-        // zeta-line (i, j) = (b, a): nodes b + SJ*a + SK*l, derivative written in place
-        double *w = sW + f * FS + el * ME + b + SJ * a;
-        line_derivs<Nq>(w, SK, w, tab);
+    // ---- phase B: line tasks (Alg. 2) ----------------------------------------------------------
+    // task (dir, f, line): buffers are laid out [sW | d/dxi | d/deta | d/dzeta], NF*FS each
+    const double *sGz = sW;
+    if constexpr (SH::POOLED) {
+        sGz = sGe + NF * FS;
+#pragma unroll 1
+        for (int T = tid; T < 3 * NF * LINES; T += SH::THREADS) {
+            const int dir = T / (NF * LINES), r = T - dir * (NF * LINES);
+            const int f = r / LINES, line = r - f * LINES;
+            if (line >= n_lines) continue;
+            const int el = (SH::EPB == 1) ? 0 : line / N2, l2 = line - el * N2;
+            const int a = l2 / Nq, b = l2 - a * Nq;  // l2 = b + Nq*a
+            // xi-line (j,k)=(b,a): l + SJ*l2;  eta-line (i,k)=(b,a): b + SJ*l + SK*a;
+            // zeta-line (i,j)=(b,a): b + SJ*a + SK*l
+            const int base = (dir == 0) ? SJ * l2 : (dir == 1) ? b + SK * a : b + SJ * a;
+            const int stride = (dir == 0) ? 1 : (dir == 1) ? SJ : SK;
+            double *src = sW + f * FS + el * ME + base;
+            line_derivs<Nq>(src, stride, src + (1 + dir) * NF * FS, tab);
+        }
+    } else {
+        // xi and eta (both only read sW), barrier, then zeta in place
+        for (int t = tid; t < NF * LINES; t += SH::THREADS) {
+            const int f = t / LINES, line = t - f * LINES;
+            if (line >= n_lines) continue;
+            const int el = (SH::EPB == 1) ? 0 : line / N2, l2 = line - el * N2;
+            const int a = l2 / Nq, b = l2 - a * Nq;
+            const int base = f * FS + el * ME;
+            line_derivs<Nq>(sW + base + SJ * l2, 1, sGx + base + SJ * l2, tab);
+            line_derivs<Nq>(sW + base + b + SK * a, SJ, sGe + base + b + SK * a, tab);
+        }
+        __syncthreads();
+        for (int t = tid; t < NF * LINES; t += SH::THREADS) {
+            const int f = t / LINES, line = t - f * LINES;
+            if (line >= n_lines) continue;
+            const int el = (SH::EPB == 1) ? 0 : line / N2, l2 = line - el * N2;
+            const int a = l2 / Nq, b = l2 - a * Nq;
+            double *w = sW + f * FS + el * ME + b + SJ * a;
+            line_derivs<Nq>(w, SK, w, tab);
+        }
     }
     __syncthreads();
     if (!has_node) return;
 
     // ---- phase C: chain rule, Eq. 1 tendencies, sources, walls, stage update (A5-A10) -------
-    double m[9];
-#pragma unroll
-    for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
-    const double om = __ldg(A.omega + p);
-    double q0v[5];
-    if (A.q0 == A.qs) {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) q0v[c] = qv[c];
-    } else {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
-    }
-    double fx[NF], fe[NF], fz[NF];
-#pragma unroll
-    for (int f = 0; f < NF; ++f) {
-        fx[f] = sGx[f * FS + sp];
-        fe[f] = sGe[f * FS + sp];
-        fz[f] = sW[f * FS + sp];
-    }
     const double rhop = qv[0], u = qv[1], v = qv[2], w = qv[3];
     const double irho = 1.0 / (rho0 + rhop);
     // contravariant velocity: u . grad f = sum_a U^a f_{xi_a}
     const double Ux = u * m[0] + v * m[1] + w * m[2];
     const double Ue = u * m[3] + v * m[4] + w * m[5];
     const double Uz = u * m[6] + v * m[7] + w * m[8];
-    const double px = fx[0] * m[0] + fe[0] * m[3] + fz[0] * m[6];
-    const double py = fx[0] * m[1] + fe[0] * m[4] + fz[0] * m[7];
-    const double pz = fx[0] * m[2] + fe[0] * m[5] + fz[0] * m[8];
+    const double *gx = sGx + sp, *ge = sGe + sp, *gz = sGz + sp;
     double S[5];
-    S[1] = -(Ux * fx[1] + Ue * fe[1] + Uz * fz[1]) - px * irho;
-    S[2] = -(Ux * fx[2] + Ue * fe[2] + Uz * fz[2]) - py * irho;
-    S[3] = -(Ux * fx[3] + Ue * fe[3] + Uz * fz[3]) - pz * irho - (rhop * irho) * A.g;
-    S[4] = -(Ux * fx[4] + Ue * fe[4] + Uz * fz[4]);
-    double div = fx[5] * m[0] + fe[5] * m[3] + fz[5] * m[6];
-    div += fx[6] * m[1] + fe[6] * m[4] + fz[6] * m[7];
-    div += fx[7] * m[2] + fe[7] * m[5] + fz[7] * m[8];
-    S[0] = -div;
+    {   // pressure gradient and buoyancy (Eq. 1b)
+        const double fx = gx[0], fe = ge[0], fz = gz[0];
+        S[1] = -(fx * m[0] + fe * m[3] + fz * m[6]) * irho;
+        S[2] = -(fx * m[1] + fe * m[4] + fz * m[7]) * irho;
+        S[3] = -(fx * m[2] + fe * m[5] + fz * m[8]) * irho - (rhop * irho) * A.g;
+    }
+#pragma unroll
+    for (int f = 1; f <= 4; ++f)  // advection of u, v, w, theta (Eq. 1b, 1c)
+        S[f] = ((f == 4) ? 0.0 : S[f]) - (Ux * gx[f * FS] + Ue * ge[f * FS] + Uz * gz[f * FS]);
+    {   // divergence of F = rho u (Eq. 1a)
+        double div = gx[5 * FS] * m[0] + ge[5 * FS] * m[3] + gz[5 * FS] * m[6];
+        div += gx[6 * FS] * m[1] + ge[6 * FS] * m[4] + gz[6 * FS] * m[7];
+        div += gx[7 * FS] * m[2] + ge[7 * FS] * m[5] + gz[7 * FS] * m[8];
+        S[0] = -div;
+    }
     // A8: heating, Coriolis, sponge
-    if (A.heat) S[4] += __ldg(A.heat + p);
+    S[4] += heat;
     S[1] += A.f_cor * v;
     S[2] -= A.f_cor * u;
-    if (A.beta) {
-        const double b = __ldg(A.beta + p);
-        S[1] -= b * u; S[2] -= b * v; S[3] -= b * w; S[4] -= b * qv[4];
-    }
+    S[1] -= beta * u; S[2] -= beta * v; S[3] -= beta * w; S[4] -= beta * qv[4];
     // A6: weight; A9: walls on the weighted velocity tendency
     double r[5];
 #pragma unroll
@@ -216,21 +251,20 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
         if (on_face) {
             const int64_t e = (p - n) / Mn;
             const uint2 bcw = *reinterpret_cast<const uint2 *>(A.face_bc + e * 8);
-            if (bcw.x | bcw.y) {
-                uint8_t bc[8];
-#pragma unroll
-                for (int f = 0; f < 4; ++f) {
-                    bc[f] = (uint8_t)(bcw.x >> (8 * f));
-                    bc[4 + f] = (uint8_t)(bcw.y >> (8 * f));
-                }
-                wall_project<Nq>(bc, i, j, k, m, r[1], r[2], r[3]);
-            }
+            if (bcw.x | bcw.y) wall_project_cold<Nq>(bcw, i, j, k, m, r[1], r[2], r[3]);
         }
     }
     // A10 as a DSS partial sum
+    double *qop = A.qout + p;
+    if (same) {
+        const double a01 = A.a0 + A.a1;
 #pragma unroll
-    for (int c = 0; c < 5; ++c)
-        A.qout[c * NL + p] = om * (A.a0 * q0v[c] + A.a1 * qv[c]) + A.b_dt * r[c];
+        for (int c = 0; c < 5; ++c) qop[c * NL] = om * (a01 * qv[c]) + A.b_dt * r[c];
+    } else {
+#pragma unroll
+        for (int c = 0; c < 5; ++c)
+            qop[c * NL] = om * (A.a0 * q0v[c] + A.a1 * qv[c]) + A.b_dt * r[c];
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -261,41 +295,28 @@ __device__ __forceinline__ void dss_node(double *r, const int32_t *__restrict__ 
     }
 }
 
-struct DssArgs {
-    const int32_t *idx;        // class lists, transposed
-    int64_t n[3], base[3];     // nodes and list offset of the classes C = 2, 4, 8
-    int64_t blk[3];            // first block of the classes 4, 8 and of the generic tail
-    const int32_t *gen_nodes;  // global ids with any other multiplicity >= 2
-    int64_t n_gen;
-    const int32_t *start, *copies;  // CSR lists (generic path)
-    int64_t NL;
-};
-
-constexpr int kDssThreads = 128;
-
-__global__ void __launch_bounds__(kDssThreads)
-k_stage_dss(double *r, const __grid_constant__ DssArgs A)
+__global__ void __launch_bounds__(NUMA_DSS_THREADS)
+k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
+            const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
+            const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL)
 {
-    const int64_t b = blockIdx.x;
-    if (b < A.blk[0]) {
-        const int64_t t = b * kDssThreads + threadIdx.x;
-        if (t < A.n[0]) dss_node<2>(r, A.idx + A.base[0], A.n[0], t, A.NL);
-    } else if (b < A.blk[1]) {
-        const int64_t t = (b - A.blk[0]) * kDssThreads + threadIdx.x;
-        if (t < A.n[1]) dss_node<4>(r, A.idx + A.base[1], A.n[1], t, A.NL);
-    } else if (b < A.blk[2]) {
-        const int64_t t = (b - A.blk[1]) * kDssThreads + threadIdx.x;
-        if (t < A.n[2]) dss_node<8>(r, A.idx + A.base[2], A.n[2], t, A.NL);
+    const DssSeg sg = segs[blkmap[blockIdx.x]];
+    const int t = (blockIdx.x - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
+    if (t >= sg.n) return;
+    if (sg.cls == 0) {
+        dss_node<2>(r, idx + sg.idx_base, sg.n, t, NL);
+    } else if (sg.cls == 1) {
+        dss_node<4>(r, idx + sg.idx_base, sg.n, t, NL);
+    } else if (sg.cls == 2) {
+        dss_node<8>(r, idx + sg.idx_base, sg.n, t, NL);
     } else {
-        const int64_t t = (b - A.blk[2]) * kDssThreads + threadIdx.x;
-        if (t >= A.n_gen) return;
-        const int gI = A.gen_nodes[t];
-        const int s = A.start[gI], c = A.start[gI + 1] - s;
+        const int gI = nodes[sg.node_off + t];
+        const int s = start[gI], c = start[gI + 1] - s;
         for (int m = 0; m < 5; ++m) {
-            double *rm = r + (int64_t)m * A.NL;
-            double sum = rm[A.copies[s]];
-            for (int a = 1; a < c; ++a) sum += rm[A.copies[s + a]];
-            for (int a = 0; a < c; ++a) rm[A.copies[s + a]] = sum;
+            double *rm = r + (int64_t)m * NL;
+            double sum = rm[copies[s]];
+            for (int a = 1; a < c; ++a) sum += rm[copies[s + a]];
+            for (int a = 0; a < c; ++a) rm[copies[s + a]] = sum;
         }
     }
 }
@@ -352,22 +373,9 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
 
 cudaError_t launch_dss_classes(numa_ctx *c, double *r, int kernel_id, cudaStream_t s)
 {
-    if (c->n_shared == 0) return cudaSuccess;
+    if (c->dss_blocks == 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
-    DssArgs a;
-    a.idx = c->dss_idx;
-    int64_t blocks = 0;
-    for (int k = 0; k < 3; ++k) {
-        a.n[k] = c->cls_n[k];
-        a.base[k] = c->cls_base[k];
-        blocks += (c->cls_n[k] + kDssThreads - 1) / kDssThreads;
-        a.blk[k] = blocks;
-    }
-    a.gen_nodes = c->gen_nodes;
-    a.n_gen = c->n_gen;
-    blocks += (c->n_gen + kDssThreads - 1) / kDssThreads;
-    a.start = c->dss_start; a.copies = c->dss_copies;
-    a.NL = c->NL;
-    k_stage_dss<<<(unsigned)blocks, kDssThreads, 0, s>>>(r, a);
+    k_stage_dss<<<(unsigned)c->dss_blocks, NUMA_DSS_THREADS, 0, s>>>(
+        r, c->dss_idx, c->dss_seg, c->dss_blkmap, c->sh_nodes, c->dss_start, c->dss_copies, c->NL);
     return cudaGetLastError();
 }
