@@ -23,8 +23,9 @@ namespace {
 // them (N+1 shared stores).  Per node and field that is 1 store + 3x(1 load + 1 store) + 3
 // loads of shared memory instead of the 3(N+1) loads of a thread-per-node contraction.
 // The zeta-derivatives overwrite the work fields in place (after a barrier), so a node needs
-// 24 doubles of shared memory.  Shared node index: i + SJ*j + SK*k, SJ odd (bank-conflict-
-// free xi-lines).
+// 24 doubles of shared memory.  Shared node index: i + SJ*j + SK*k.  Line tasks are numbered
+// field-fastest and the field stride is 2 (mod 4) doubles, which makes every line access of a
+// half-warp hit 16 distinct banks (StageShape).
 // ---------------------------------------------------------------------------------------
 template <int N>
 struct StageShape {
@@ -36,14 +37,24 @@ struct StageShape {
 #define STAGE_MINB4 6
 #endif
     static constexpr int EPB = (N == 2) ? 9 : (N == 3) ? 4 : (N == 4) ? STAGE_EPB4 : 1;
-    static constexpr int SJ = (Nq & 1) ? Nq : Nq + 1;
-    static constexpr int SK = SJ * Nq;
+    // shared node index i + SJ*j + SK*k; for even Nq the k-planes are padded by one double
+    static constexpr int SJ = Nq;
+    static constexpr int SK = (Nq & 1) ? N2 : N2 + 1;
     static constexpr int ME = SK * Nq;  // padded nodes per element and field
     static constexpr int NF = 8;        // p', u, v, w, theta, Fx, Fy, Fz
     static constexpr int NODES = EPB * Mn;
+    // Thread t of a block works on node  align_down(node0, 16) + t  (wrapping around inside the
+    // block's THREADS-node window), so that every warp-wide 8-byte global access starts on a
+    // 128-byte line: two L1 wavefronts instead of four to five when (N+1)^3 is not a multiple
+    // of 16.  WRAP = whether node0 can be misaligned at all.
+    static constexpr bool WRAP = (NODES % 16) != 0;
     static constexpr int THREADS = (NODES + 31) / 32 * 32;
     static constexpr int LINES = EPB * N2;  // lines per field and direction
-    static constexpr int FS = EPB * ME;     // field stride in shared memory
+    // field stride in shared memory: = 2 (mod 4) doubles, so that with the FIELD-FASTEST task
+    // enumeration (lane -> field = T mod 8, line = T / 8) the 16 lanes of a half-warp hit 16
+    // different 8-byte banks in all three line directions (brute-forced).
+    static constexpr int FS = EPB * ME + ((EPB * ME) % 4 == 2 ? 0 : (EPB * ME) % 4 == 1 ? 1
+                            : (EPB * ME) % 4 == 0 ? 2 : 3);
     // POOLED: the zeta-derivatives get their own buffer, so the line tasks of all three
     // directions form one pool without a barrier in between (better balance at low N);
     // otherwise they overwrite the work fields in place after a barrier (less shared memory).
@@ -130,12 +141,15 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     const int n_nodes = rem < SH::NODES ? (int)rem : SH::NODES;  // ragged last block
     const int n_lines = n_nodes / Nq;                            // = elements * N2
 
-    // this thread's node (pointwise role)
-    const bool has_node = tid < n_nodes;
-    const int le = tid / Mn, n = tid - le * Mn;
+    // this thread's node (pointwise role): threads are laid over the 16-node-aligned window
+    // that starts at or before node0; the threads in front of node0 take the window's tail
+    int bn = tid - (SH::WRAP ? (int)(node0 & 15) : 0);  // node within the block
+    if (SH::WRAP && bn < 0) bn += SH::THREADS;
+    const bool has_node = bn < n_nodes;
+    const int le = has_node ? bn / Mn : 0, n = has_node ? bn - le * Mn : 0;
     const int k = n / N2, j = (n - k * N2) / Nq, i = n - k * N2 - j * Nq;
     const int sp = le * ME + i + SJ * j + SK * k;
-    const int64_t p = node0 + tid;
+    const int64_t p = node0 + bn;
 
     // ---- phase A: pointwise pre-pass (A2) ---------------------------------------------------
     double qv[5] = {0, 0, 0, 0, 0}, rho0 = 1.0;
@@ -171,20 +185,23 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     __syncthreads();
 
     // ---- phase B: line tasks (Alg. 2) ----------------------------------------------------------
-    // task (dir, f, line): buffers are laid out [sW | d/dxi | d/deta | d/dzeta], NF*FS each
+    // Task t -> field f = t mod 8 (fastest), line = t / 8 = l2 + N2*element, l2 = lo + Nq*hi.
+    //   xi-line:   odd Nq (j,k) = (lo,hi), even Nq (j,k) = (hi,lo);  points l + SJ*j + SK*k
+    //   eta-line:  (i,k) = (lo,hi);  points i + SJ*l + SK*k
+    //   zeta-line: (i,j) = (lo,hi);  points i + SJ*j + SK*l
+    // buffers are laid out [sW | d/dxi | d/deta | d/dzeta], NF*FS each
     const double *sGz = sW;
     if constexpr (SH::POOLED) {
         sGz = sGe + NF * FS;
 #pragma unroll 1
         for (int T = tid; T < 3 * NF * LINES; T += SH::THREADS) {
             const int dir = T / (NF * LINES), r = T - dir * (NF * LINES);
-            const int f = r / LINES, line = r - f * LINES;
+            const int f = r & 7, line = r >> 3;
             if (line >= n_lines) continue;
             const int el = (SH::EPB == 1) ? 0 : line / N2, l2 = line - el * N2;
-            const int a = l2 / Nq, b = l2 - a * Nq;  // l2 = b + Nq*a
-            // xi-line (j,k)=(b,a): l + SJ*l2;  eta-line (i,k)=(b,a): b + SJ*l + SK*a;
-            // zeta-line (i,j)=(b,a): b + SJ*a + SK*l
-            const int base = (dir == 0) ? SJ * l2 : (dir == 1) ? b + SK * a : b + SJ * a;
+            const int hi = l2 / Nq, lo = l2 - hi * Nq;
+            const int bx = (Nq & 1) ? SJ * lo + SK * hi : SJ * hi + SK * lo;
+            const int base = (dir == 0) ? bx : (dir == 1) ? lo + SK * hi : lo + SJ * hi;
             const int stride = (dir == 0) ? 1 : (dir == 1) ? SJ : SK;
             double *src = sW + f * FS + el * ME + base;
             line_derivs<Nq>(src, stride, src + (1 + dir) * NF * FS, tab);
@@ -192,21 +209,22 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     } else {
         // xi and eta (both only read sW), barrier, then zeta in place
         for (int t = tid; t < NF * LINES; t += SH::THREADS) {
-            const int f = t / LINES, line = t - f * LINES;
+            const int f = t & 7, line = t >> 3;
             if (line >= n_lines) continue;
             const int el = (SH::EPB == 1) ? 0 : line / N2, l2 = line - el * N2;
-            const int a = l2 / Nq, b = l2 - a * Nq;
+            const int hi = l2 / Nq, lo = l2 - hi * Nq;
             const int base = f * FS + el * ME;
-            line_derivs<Nq>(sW + base + SJ * l2, 1, sGx + base + SJ * l2, tab);
-            line_derivs<Nq>(sW + base + b + SK * a, SJ, sGe + base + b + SK * a, tab);
+            const int bx = base + ((Nq & 1) ? SJ * lo + SK * hi : SJ * hi + SK * lo);
+            line_derivs<Nq>(sW + bx, 1, sGx + bx, tab);
+            line_derivs<Nq>(sW + base + lo + SK * hi, SJ, sGe + base + lo + SK * hi, tab);
         }
         __syncthreads();
         for (int t = tid; t < NF * LINES; t += SH::THREADS) {
-            const int f = t / LINES, line = t - f * LINES;
+            const int f = t & 7, line = t >> 3;
             if (line >= n_lines) continue;
             const int el = (SH::EPB == 1) ? 0 : line / N2, l2 = line - el * N2;
-            const int a = l2 / Nq, b = l2 - a * Nq;
-            double *w = sW + f * FS + el * ME + b + SJ * a;
+            const int hi = l2 / Nq, lo = l2 - hi * Nq;
+            double *w = sW + f * FS + el * ME + lo + SJ * hi;
             line_derivs<Nq>(w, SK, w, tab);
         }
     }
@@ -274,28 +292,25 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 // values are loaded before the first store.  Sum in ascending local index.
 // ---------------------------------------------------------------------------------------
 template <int C>
-__device__ __forceinline__ void dss_node(double *r, const int32_t *__restrict__ idx, int64_t n,
-                                         int64_t t, int64_t NL)
+__device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__ idx, int64_t n,
+                                         int64_t t)
 {
     int32_t id[C];
 #pragma unroll
     for (int a = 0; a < C; ++a) id[a] = idx[a * n + t];
-    double v[5][C];
+    double v[C];
 #pragma unroll
-    for (int m = 0; m < 5; ++m)
+    for (int a = 0; a < C; ++a) v[a] = rm[id[a]];
+    double s = v[0];
 #pragma unroll
-        for (int a = 0; a < C; ++a) v[m][a] = r[m * NL + id[a]];
+    for (int a = 1; a < C; ++a) s += v[a];
 #pragma unroll
-    for (int m = 0; m < 5; ++m) {
-        double s = v[m][0];
-#pragma unroll
-        for (int a = 1; a < C; ++a) s += v[m][a];
-#pragma unroll
-        for (int a = 0; a < C; ++a) r[m * NL + id[a]] = s;
-    }
+    for (int a = 0; a < C; ++a) rm[id[a]] = s;
 }
 
-__global__ void __launch_bounds__(NUMA_DSS_THREADS)
+// block = (NUMA_DSS_THREADS shared nodes) x (5 fields): few registers per thread, so the SM
+// holds its full 2048 threads of independent gathers (the kernel is latency-bound).
+__global__ void __launch_bounds__(NUMA_DSS_THREADS * 5)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
             const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
             const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL)
@@ -303,21 +318,19 @@ k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict
     const DssSeg sg = segs[blkmap[blockIdx.x]];
     const int t = (blockIdx.x - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
     if (t >= sg.n) return;
+    double *rm = r + (int64_t)threadIdx.y * NL;
     if (sg.cls == 0) {
-        dss_node<2>(r, idx + sg.idx_base, sg.n, t, NL);
+        dss_node<2>(rm, idx + sg.idx_base, sg.n, t);
     } else if (sg.cls == 1) {
-        dss_node<4>(r, idx + sg.idx_base, sg.n, t, NL);
+        dss_node<4>(rm, idx + sg.idx_base, sg.n, t);
     } else if (sg.cls == 2) {
-        dss_node<8>(r, idx + sg.idx_base, sg.n, t, NL);
+        dss_node<8>(rm, idx + sg.idx_base, sg.n, t);
     } else {
         const int gI = nodes[sg.node_off + t];
         const int s = start[gI], c = start[gI + 1] - s;
-        for (int m = 0; m < 5; ++m) {
-            double *rm = r + (int64_t)m * NL;
-            double sum = rm[copies[s]];
-            for (int a = 1; a < c; ++a) sum += rm[copies[s + a]];
-            for (int a = 0; a < c; ++a) rm[copies[s + a]] = sum;
-        }
+        double sum = rm[copies[s]];
+        for (int a = 1; a < c; ++a) sum += rm[copies[s + a]];
+        for (int a = 0; a < c; ++a) rm[copies[s + a]] = sum;
     }
 }
 
@@ -375,7 +388,7 @@ cudaError_t launch_dss_classes(numa_ctx *c, double *r, int kernel_id, cudaStream
 {
     if (c->dss_blocks == 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
-    k_stage_dss<<<(unsigned)c->dss_blocks, NUMA_DSS_THREADS, 0, s>>>(
+    k_stage_dss<<<(unsigned)c->dss_blocks, dim3(NUMA_DSS_THREADS, 5), 0, s>>>(
         r, c->dss_idx, c->dss_seg, c->dss_blkmap, c->sh_nodes, c->dss_start, c->dss_copies, c->NL);
     return cudaGetLastError();
 }
