@@ -59,11 +59,33 @@ struct StageShape {
     // directions form one pool without a barrier in between (better balance at low N);
     // otherwise they overwrite the work fields in place after a barrier (less shared memory).
 #ifndef STAGE_POOLED_MAXN
-#define STAGE_POOLED_MAXN 3
+#define STAGE_POOLED_MAXN 2
 #endif
     static constexpr bool POOLED = (N <= STAGE_POOLED_MAXN);
     static constexpr size_t SMEM = sizeof(double) * (POOLED ? 4 : 3) * NF * FS;
-    static constexpr int MIN_BLOCKS = (N == 4) ? STAGE_MINB4 : (N < 4) ? 3 : (N <= 6) ? 2 : 1;
+    // PREFETCH: request the phase-C inputs in phase A (17 doubles live across phase B); at high
+    // N the registers are worth more as a second resident block.
+#ifndef STAGE_PREFETCH_MAXN
+#define STAGE_PREFETCH_MAXN 5
+#endif
+    static constexpr bool PREFETCH = (N <= STAGE_PREFETCH_MAXN);
+#ifndef STAGE_MINB3
+#define STAGE_MINB3 3
+#endif
+#ifndef STAGE_MINB5
+#define STAGE_MINB5 4
+#endif
+#ifndef STAGE_MINB6
+#define STAGE_MINB6 2
+#endif
+#ifndef STAGE_MINB7
+#define STAGE_MINB7 1
+#endif
+#ifndef STAGE_MINB8
+#define STAGE_MINB8 1
+#endif
+    static constexpr int MIN_BLOCKS = (N == 4) ? STAGE_MINB4 : (N == 3) ? STAGE_MINB3 : (N == 5) ? STAGE_MINB5
+                                    : (N == 6) ? STAGE_MINB6 : (N == 7) ? STAGE_MINB7 : (N == 8) ? STAGE_MINB8 : 3;
 };
 
 struct StageArgs {
@@ -159,15 +181,17 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     if (has_node) {
 #pragma unroll
         for (int c = 0; c < 5; ++c) qv[c] = A.qs[c * NL + p];
+        if constexpr (SH::PREFETCH) {
 #pragma unroll
-        for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
-        om = __ldg(A.omega + p);
-        if (!same) {
+            for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
+            om = __ldg(A.omega + p);
+            if (!same) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+                for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+            }
+            if (A.heat) heat = __ldg(A.heat + p);
+            if (A.beta) beta = __ldg(A.beta + p);
         }
-        if (A.heat) heat = __ldg(A.heat + p);
-        if (A.beta) beta = __ldg(A.beta + p);
         rho0 = __ldg(A.ref3 + p);
         const double th0 = __ldg(A.ref3 + NL + p), p0 = __ldg(A.ref3 + 2 * NL + p);
         const double th0e = __ldg(A.ref3 + NL + (p - n));  // theta0 at the element's first node (Q7)
@@ -232,6 +256,17 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     if (!has_node) return;
 
     // ---- phase C: chain rule, Eq. 1 tendencies, sources, walls, stage update (A5-A10) -------
+    if constexpr (!SH::PREFETCH) {
+#pragma unroll
+        for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
+        om = __ldg(A.omega + p);
+        if (!same) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+        }
+        if (A.heat) heat = __ldg(A.heat + p);
+        if (A.beta) beta = __ldg(A.beta + p);
+    }
     const double rhop = qv[0], u = qv[1], v = qv[2], w = qv[3];
     const double irho = 1.0 / (rho0 + rhop);
     // contravariant velocity: u . grad f = sum_a U^a f_{xi_a}
