@@ -131,9 +131,10 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
 
 // A9 for the few nodes that lie on a wall face: kept out of line so that its square roots
 // and divisions do not weigh on the registers and code of the common path.
+struct WallIO { double m[9]; double r[3]; };
+
 template <int Nq>
-__device__ __noinline__ void wall_project_cold(uint2 bcw, int i, int j, int k, const double (&m)[9],
-                                               double &ru, double &rv, double &rw)
+__device__ __noinline__ void wall_project_cold(uint2 bcw, int i, int j, int k, WallIO *io)
 {
     uint8_t bc[8];
 #pragma unroll
@@ -141,7 +142,7 @@ __device__ __noinline__ void wall_project_cold(uint2 bcw, int i, int j, int k, c
         bc[f] = (uint8_t)(bcw.x >> (8 * f));
         bc[4 + f] = (uint8_t)(bcw.y >> (8 * f));
     }
-    wall_project<Nq>(bc, i, j, k, m, ru, rv, rw);
+    wall_project<Nq>(bc, i, j, k, io->m, io->r[0], io->r[1], io->r[2]);
 }
 
 template <int N>
@@ -304,7 +305,16 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
         if (on_face) {
             const int64_t e = (p - n) / Mn;
             const uint2 bcw = *reinterpret_cast<const uint2 *>(A.face_bc + e * 8);
-            if (bcw.x | bcw.y) wall_project_cold<Nq>(bcw, i, j, k, m, r[1], r[2], r[3]);
+            if (bcw.x | bcw.y) {
+                // copies made only on this rare path: the out-of-line call needs its operands in
+                // local memory, and m[] / r[] themselves must stay in registers for everyone else
+                WallIO io;
+#pragma unroll
+                for (int c = 0; c < 9; ++c) io.m[c] = m[c];
+                io.r[0] = r[1]; io.r[1] = r[2]; io.r[2] = r[3];
+                wall_project_cold<Nq>(bcw, i, j, k, &io);
+                r[1] = io.r[0]; r[2] = io.r[1]; r[3] = io.r[2];
+            }
         }
     }
     // A10 as a DSS partial sum
