@@ -143,6 +143,22 @@ def time_oracle(wl, steps, warmup):
     return t, cores
 
 
+def max_over_ranks(x, device, world):
+    """MAX over ranks of one float (torch.distributed must be initialised when world > 1)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gdof_per_s(n_local, steps, world, seconds):
+    """Whole-job value: every rank (replica) advances n_local nodes x 5 DOF x 3 stages per step."""
+    return 5.0 * n_local * 3 * steps * world / seconds / 1e9
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on a bounded sample (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -221,10 +237,7 @@ def run_gpu(args):
     g.profile(False)
     clocks = sampler.stop() if rank == 0 else None
     finite = bool(torch.isfinite(q).all().item())
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dev, world)
 
     # ---- end to end through the C ABI with host buffers ---------------------------------
     qh = torch.from_numpy(wl.q.copy()).pin_memory()
@@ -239,10 +252,7 @@ def run_gpu(args):
         g.step_rk3_host(qh, wl.dt, hh, 1, dq, dh)   # H2D state+heating, 1 step, D2H state, sync
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_e2e = float(t.item())
+    t_e2e = max_over_ranks(t_e2e, dev, world)
     h2d = 5 * NL * 8 + (NL * 8 if hh is not None else 0)
     d2h = 5 * NL * 8
 
@@ -251,9 +261,8 @@ def run_gpu(args):
             dist.destroy_process_group()
         return
 
-    dof_evals = 5.0 * NL * 3 * args.steps * world
-    value = dof_evals / (ms * 1e-3) / 1e9
-    e2e_value = 5.0 * NL * 3 * e2e_steps * world / t_e2e / 1e9
+    value = whole_job_gdof_per_s(NL, args.steps, world, ms * 1e-3)
+    e2e_value = whole_job_gdof_per_s(NL, e2e_steps, world, t_e2e)
 
     # ---- roofline of the dominant kernel -------------------------------------------------
     peak, peak_src = measured_peaks()

@@ -339,3 +339,37 @@ def test_host_buffer_entry_point_matches_device_path():
     hh = torch.from_numpy(wl.heating.copy()).pin_memory()
     g.step_rk3_host(qh, wl.dt, hh, 2)
     assert torch.equal(qh, qd.cpu())
+
+
+def test_full_size_cfg3_in_the_bench_configuration():
+    """The workload and launch configuration bench.py times by default (config 3: 100x100x20
+    elements, N=4, 25 M local nodes, heating + sponge + Coriolis + walls): one full RHS through
+    the four C-ABI calls and two fused SSP-RK3 steps, against the oracle element by element at
+    full size (the oracle needs ~1 min and ~10 GB of host memory for this)."""
+    wl = inputs.make_workload(3)
+    assert wl.mesh.n_local == 25_000_000
+    o, g = _pair(wl)
+    hd = g.state(wl.heating)
+    # one RHS evaluation (four-call route) on the workload's initial state
+    r_o = o.rhs(wl.q, wl.heating)
+    T = _assembled_T(o, wl.q)
+    r_g = _np(g.full_rhs(g.state(wl.q), hd))
+    e = rel_l2(r_g, r_o, T)
+    assert np.all(e <= TOL_RHS), describe(r_g, r_o, T)
+    del r_g, r_o, T
+    # two steps of the fused route (six stages)
+    qd = g.state(wl.q)
+    g.step_rk3(qd, wl.dt, hd, 2)
+    q = wl.q
+    for _ in range(2):
+        q = o.step_rk3(q, wl.dt, wl.heating)
+    qg = _np(qd)
+    e = rel_l2(qg, q)
+    assert np.all(e <= TOL_RHS * 6), e      # six stages, each within the per-call tolerance
+    # copies of a global node are bitwise equal after the in-place DSS, at full size
+    cg = wl.mesh.intma_cg.reshape(-1)
+    first = np.full(wl.mesh.n_global, -1, dtype=np.int64)
+    first[cg[::-1]] = np.arange(cg.size - 1, -1, -1)
+    for m in range(5):
+        f = qg[m].reshape(-1)
+        assert np.array_equal(f, f[first[cg]])
