@@ -48,7 +48,18 @@ struct StageShape {
     // 128-byte line: two L1 wavefronts instead of four to five when (N+1)^3 is not a multiple
     // of 16.  WRAP = whether node0 can be misaligned at all.
     static constexpr bool WRAP = (NODES % 16) != 0;
-    static constexpr int THREADS = (NODES + 31) / 32 * 32;
+    // NPT nodes per thread in the pointwise phases: at high N a block of Mn threads would be
+    // alone on its SM (registers, shared memory); half as many threads let two blocks overlap
+    // their memory and compute phases.
+#ifndef STAGE_NPT_HI
+#define STAGE_NPT_HI 2
+#endif
+#ifndef STAGE_NPT_MINN
+#define STAGE_NPT_MINN 9  /* measured: no gain at N <= 8; kept for larger elements */
+#endif
+    static constexpr int NPT = (N >= STAGE_NPT_MINN) ? STAGE_NPT_HI : 1;
+    static constexpr int THREADS = ((NODES + NPT - 1) / NPT + 31) / 32 * 32;
+    static constexpr int SLOTS = THREADS * NPT;  // >= NODES
     static constexpr int LINES = EPB * N2;  // lines per field and direction
     // field stride in shared memory: = 2 (mod 4) doubles, so that with the FIELD-FASTEST task
     // enumeration (lane -> field = T mod 8, line = T / 8) the 16 lanes of a half-warp hit 16
@@ -62,13 +73,21 @@ struct StageShape {
 #define STAGE_POOLED_MAXN 2
 #endif
     static constexpr bool POOLED = (N <= STAGE_POOLED_MAXN);
-    static constexpr size_t SMEM = sizeof(double) * (POOLED ? 4 : 3) * NF * FS;
+    static constexpr size_t SMEM_WORK = sizeof(double) * (POOLED ? 4 : 3) * NF * FS;
     // PREFETCH: request the phase-C inputs in phase A (17 doubles live across phase B); at high
     // N the registers are worth more as a second resident block.
 #ifndef STAGE_PREFETCH_MAXN
 #define STAGE_PREFETCH_MAXN 5
 #endif
     static constexpr bool PREFETCH = (N <= STAGE_PREFETCH_MAXN);
+    // PFS: the same 17 inputs are prefetched with cp.async into shared memory instead (no
+    // registers held across phase B); used where one block per SM leaves the room (N = 6, 7).
+#ifndef STAGE_PFS_MASK
+#define STAGE_PFS_MASK 0x80  /* bit N set = use it (measured: pays at N = 7 only) */
+#endif
+    static constexpr bool PFS = !PREFETCH && ((STAGE_PFS_MASK >> N) & 1);
+    static constexpr int NPF = 17;  // met[9], omega, q0[5], heat, beta
+    static constexpr size_t SMEM = SMEM_WORK + (PFS ? sizeof(double) * NPF * SLOTS : 0);
 #ifndef STAGE_MINB3
 #define STAGE_MINB3 3
 #endif
@@ -145,6 +164,34 @@ __device__ __noinline__ void wall_project_cold(uint2 bcw, int i, int j, int k, W
     wall_project<Nq>(bc, i, j, k, io->m, io->r[0], io->r[1], io->r[2]);
 }
 
+__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+
+// Pointwise role of a thread: slot -> node.  The SLOTS slots of a block are laid over the
+// 16-node-aligned window that starts at or before node0; the slots in front of node0 take the
+// window's tail.
+struct NodeIx { bool has; int n, i, j, k, sp; int64_t p; };
+
+template <class SH>
+__device__ __forceinline__ NodeIx node_ix(int slot, int64_t node0, int n_nodes)
+{
+    int bn = slot - (SH::WRAP ? (int)(node0 & 15) : 0);  // node within the block
+    if (SH::WRAP && bn < 0) bn += SH::SLOTS;
+    NodeIx x;
+    x.has = bn < n_nodes;
+    const int le = x.has ? bn / SH::Mn : 0;
+    x.n = x.has ? bn - le * SH::Mn : 0;
+    x.k = x.n / SH::N2;
+    x.j = (x.n - x.k * SH::N2) / SH::Nq;
+    x.i = x.n - x.k * SH::N2 - x.j * SH::Nq;
+    x.sp = le * SH::ME + x.i + SH::SJ * x.j + SH::SK * x.k;
+    x.p = node0 + bn;
+    return x;
+}
+
 template <int N>
 __global__ void __launch_bounds__(StageShape<N>::THREADS, StageShape<N>::MIN_BLOCKS)
 k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglTables tab)
@@ -156,6 +203,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     double *sW = smem;            // [NF][EPB][ME] nodal work fields, later d/dzeta
     double *sGx = sW + NF * FS;   // d/dxi
     double *sGe = sGx + NF * FS;  // d/deta
+    double *sPF = smem + SH::SMEM_WORK / sizeof(double);  // [NPF][SLOTS] cp.async prefetch (PFS)
 
     const int tid = threadIdx.x;
     const int64_t NL = A.NL;
@@ -164,24 +212,39 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     const int n_nodes = rem < SH::NODES ? (int)rem : SH::NODES;  // ragged last block
     const int n_lines = n_nodes / Nq;                            // = elements * N2
 
-    // this thread's node (pointwise role): threads are laid over the 16-node-aligned window
-    // that starts at or before node0; the threads in front of node0 take the window's tail
-    int bn = tid - (SH::WRAP ? (int)(node0 & 15) : 0);  // node within the block
-    if (SH::WRAP && bn < 0) bn += SH::THREADS;
-    const bool has_node = bn < n_nodes;
-    const int le = has_node ? bn / Mn : 0, n = has_node ? bn - le * Mn : 0;
-    const int k = n / N2, j = (n - k * N2) / Nq, i = n - k * N2 - j * Nq;
-    const int sp = le * ME + i + SJ * j + SK * k;
-    const int64_t p = node0 + bn;
+    constexpr int NPT = SH::NPT;
+    static_assert(!SH::PREFETCH || NPT == 1, "register prefetch only with one node per thread");
 
     // ---- phase A: pointwise pre-pass (A2) ---------------------------------------------------
-    double qv[5] = {0, 0, 0, 0, 0}, rho0 = 1.0;
+    double qv[NPT][5], rho0[NPT];
     // inputs of phase C, requested now so that they are in flight during phases A and B
     double m[9], q0v[5], om = 0.0, heat = 0.0, beta = 0.0;
     const bool same = (A.q0 == A.qs);
-    if (has_node) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) qv[c] = A.qs[c * NL + p];
+    for (int rr = 0; rr < NPT; ++rr) {
+        const NodeIx x = node_ix<SH>(tid + rr * SH::THREADS, node0, n_nodes);
+        const int64_t p = x.p;
+        const int sp = x.sp;
+        rho0[rr] = 1.0;
+#pragma unroll
+        for (int c = 0; c < 5; ++c) qv[rr][c] = 0.0;
+        if (!x.has) continue;
+        if constexpr (SH::PFS) {
+            // phase-C inputs of this node -> shared memory, asynchronously; only this thread
+            // reads them back, so cp.async.wait_group is all the synchronisation needed
+            double *d = sPF + (tid + rr * SH::THREADS);
+#pragma unroll
+            for (int c = 0; c < 9; ++c) cp_async8(d + c * SH::SLOTS, A.met + c * NL + p);
+            cp_async8(d + 9 * SH::SLOTS, A.omega + p);
+            if (!same) {
+#pragma unroll
+                for (int c = 0; c < 5; ++c) cp_async8(d + (10 + c) * SH::SLOTS, A.q0 + c * NL + p);
+            }
+            if (A.heat) cp_async8(d + 15 * SH::SLOTS, A.heat + p);
+            if (A.beta) cp_async8(d + 16 * SH::SLOTS, A.beta + p);
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) qv[rr][c] = A.qs[c * NL + p];
         if constexpr (SH::PREFETCH) {
 #pragma unroll
             for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
@@ -193,20 +256,21 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
             if (A.heat) heat = __ldg(A.heat + p);
             if (A.beta) beta = __ldg(A.beta + p);
         }
-        rho0 = __ldg(A.ref3 + p);
+        rho0[rr] = __ldg(A.ref3 + p);
         const double th0 = __ldg(A.ref3 + NL + p), p0 = __ldg(A.ref3 + 2 * NL + p);
-        const double th0e = __ldg(A.ref3 + NL + (p - n));  // theta0 at the element's first node (Q7)
-        const double x = (qv[0] * th0 + qv[4] * rho0 + qv[0] * qv[4]) / (rho0 * th0);
-        const double rho = rho0 + qv[0];
-        sW[0 * FS + sp] = p0 * eos_ratio(x, A.gamma, A.eos);
-        sW[1 * FS + sp] = qv[1];
-        sW[2 * FS + sp] = qv[2];
-        sW[3 * FS + sp] = qv[3];
-        sW[4 * FS + sp] = qv[4] + (th0 - th0e);
-        sW[5 * FS + sp] = rho * qv[1];
-        sW[6 * FS + sp] = rho * qv[2];
-        sW[7 * FS + sp] = rho * qv[3];
+        const double th0e = __ldg(A.ref3 + NL + (p - x.n));  // theta0 at the element's first node (Q7)
+        const double xx = (qv[rr][0] * th0 + qv[rr][4] * rho0[rr] + qv[rr][0] * qv[rr][4]) / (rho0[rr] * th0);
+        const double rho = rho0[rr] + qv[rr][0];
+        sW[0 * FS + sp] = p0 * eos_ratio(xx, A.gamma, A.eos);
+        sW[1 * FS + sp] = qv[rr][1];
+        sW[2 * FS + sp] = qv[rr][2];
+        sW[3 * FS + sp] = qv[rr][3];
+        sW[4 * FS + sp] = qv[rr][4] + (th0 - th0e);
+        sW[5 * FS + sp] = rho * qv[rr][1];
+        sW[6 * FS + sp] = rho * qv[rr][2];
+        sW[7 * FS + sp] = rho * qv[rr][3];
     }
+    if constexpr (SH::PFS) asm volatile("cp.async.commit_group;" ::: "memory");
     __syncthreads();
 
     // ---- phase B: line tasks (Alg. 2) ----------------------------------------------------------
@@ -254,10 +318,27 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
         }
     }
     __syncthreads();
-    if (!has_node) return;
 
     // ---- phase C: chain rule, Eq. 1 tendencies, sources, walls, stage update (A5-A10) -------
-    if constexpr (!SH::PREFETCH) {
+#pragma unroll
+    for (int rr = 0; rr < NPT; ++rr) {
+    const NodeIx x = node_ix<SH>(tid + rr * SH::THREADS, node0, n_nodes);
+    if (!x.has) continue;
+    const int64_t p = x.p;
+    const int sp = x.sp, n = x.n, i = x.i, j = x.j, k = x.k;
+    if constexpr (SH::PFS) {
+        if (rr == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
+        const double *d = sPF + (tid + rr * SH::THREADS);
+#pragma unroll
+        for (int c = 0; c < 9; ++c) m[c] = d[c * SH::SLOTS];
+        om = d[9 * SH::SLOTS];
+        if (!same) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) q0v[c] = d[(10 + c) * SH::SLOTS];
+        }
+        heat = A.heat ? d[15 * SH::SLOTS] : 0.0;
+        beta = A.beta ? d[16 * SH::SLOTS] : 0.0;
+    } else if constexpr (!SH::PREFETCH) {
 #pragma unroll
         for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
         om = __ldg(A.omega + p);
@@ -265,11 +346,11 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 #pragma unroll
             for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
         }
-        if (A.heat) heat = __ldg(A.heat + p);
-        if (A.beta) beta = __ldg(A.beta + p);
+        heat = A.heat ? __ldg(A.heat + p) : 0.0;
+        beta = A.beta ? __ldg(A.beta + p) : 0.0;
     }
-    const double rhop = qv[0], u = qv[1], v = qv[2], w = qv[3];
-    const double irho = 1.0 / (rho0 + rhop);
+    const double rhop = qv[rr][0], u = qv[rr][1], v = qv[rr][2], w = qv[rr][3];
+    const double irho = 1.0 / (rho0[rr] + rhop);
     // contravariant velocity: u . grad f = sum_a U^a f_{xi_a}
     const double Ux = u * m[0] + v * m[1] + w * m[2];
     const double Ue = u * m[3] + v * m[4] + w * m[5];
@@ -295,7 +376,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     S[4] += heat;
     S[1] += A.f_cor * v;
     S[2] -= A.f_cor * u;
-    S[1] -= beta * u; S[2] -= beta * v; S[3] -= beta * w; S[4] -= beta * qv[4];
+    S[1] -= beta * u; S[2] -= beta * v; S[3] -= beta * w; S[4] -= beta * qv[rr][4];
     // A6: weight; A9: walls on the weighted velocity tendency
     double r[5];
 #pragma unroll
@@ -322,12 +403,13 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     if (same) {
         const double a01 = A.a0 + A.a1;
 #pragma unroll
-        for (int c = 0; c < 5; ++c) qop[c * NL] = om * (a01 * qv[c]) + A.b_dt * r[c];
+        for (int c = 0; c < 5; ++c) qop[c * NL] = om * (a01 * qv[rr][c]) + A.b_dt * r[c];
     } else {
 #pragma unroll
         for (int c = 0; c < 5; ++c)
-            qop[c * NL] = om * (A.a0 * q0v[c] + A.a1 * qv[c]) + A.b_dt * r[c];
+            qop[c * NL] = om * (A.a0 * q0v[c] + A.a1 * qv[rr][c]) + A.b_dt * r[c];
     }
+    }  // rr
 }
 
 // ---------------------------------------------------------------------------------------
