@@ -184,7 +184,11 @@ __global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *_
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
         const int32_t g = nodes[t];
         const int32_t s = start[g], c = start[g + 1] - s;
+#ifdef NUMA_DSS_NOCLASS
+        const uint64_t cls = 3;
+#else
         const uint64_t cls = (c == 2) ? 0 : (c == 4) ? 1 : (c == 8) ? 2 : 3;
+#endif
         const uint32_t first = (uint32_t)copies[s];
         keys[t] = ((uint64_t)(first / NUMA_DSS_CHUNK) << 34) | (cls << 32) | first;
     }

@@ -21,7 +21,7 @@ enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_F
 
 #define NUMA_DSS_CHUNK 32768   // local nodes per DSS locality chunk
 #ifndef NUMA_DSS_THREADS
-#define NUMA_DSS_THREADS 128   // shared nodes per thread block of the DSS kernel
+#define NUMA_DSS_THREADS 64    // shared nodes per thread block of the DSS kernel
 #endif
 
 struct DssSeg {

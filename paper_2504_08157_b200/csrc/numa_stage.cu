@@ -418,46 +418,70 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 // (idx[a*n + t]) so that the index loads coalesce and carry no dependent chain; all 5*C
 // values are loaded before the first store.  Sum in ascending local index.
 // ---------------------------------------------------------------------------------------
-template <int C>
+#ifndef NUMA_DSS_FPT
+#define NUMA_DSS_FPT 5   // fields per thread: 1 (block = nodes x 5 fields) or 5
+#endif
+
+// the copies are touched once per launch by this SM: keep them out of L1 (ld/st .cg)
+#if !defined(NUMA_DSS_CA) && !defined(NUMA_DSS_CS)
+#define DSS_LD(p) __ldcg(p)
+#define DSS_ST(p, v) __stcg(p, v)
+#elif defined(NUMA_DSS_CS)
+#define DSS_LD(p) __ldcs(p)
+#define DSS_ST(p, v) __stcs(p, v)
+#else
+#define DSS_LD(p) (*(p))
+#define DSS_ST(p, v) (*(p) = (v))
+#endif
+
+template <int C, int F>
 __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__ idx, int64_t n,
-                                         int64_t t)
+                                         int64_t t, int64_t NL)
 {
     int32_t id[C];
 #pragma unroll
     for (int a = 0; a < C; ++a) id[a] = idx[a * n + t];
-    double v[C];
+    double v[F][C];
 #pragma unroll
-    for (int a = 0; a < C; ++a) v[a] = rm[id[a]];
-    double s = v[0];
+    for (int m = 0; m < F; ++m)
 #pragma unroll
-    for (int a = 1; a < C; ++a) s += v[a];
+        for (int a = 0; a < C; ++a) v[m][a] = DSS_LD(rm + m * NL + id[a]);
 #pragma unroll
-    for (int a = 0; a < C; ++a) rm[id[a]] = s;
+    for (int m = 0; m < F; ++m) {
+        double s = v[m][0];
+#pragma unroll
+        for (int a = 1; a < C; ++a) s += v[m][a];
+#pragma unroll
+        for (int a = 0; a < C; ++a) DSS_ST(rm + m * NL + id[a], s);
+    }
 }
 
-// block = (NUMA_DSS_THREADS shared nodes) x (5 fields): few registers per thread, so the SM
-// holds its full 2048 threads of independent gathers (the kernel is latency-bound).
-__global__ void __launch_bounds__(NUMA_DSS_THREADS * 5)
+// block = (NUMA_DSS_THREADS shared nodes) x (5 / NUMA_DSS_FPT field groups)
+__global__ void __launch_bounds__(NUMA_DSS_THREADS * (5 / NUMA_DSS_FPT))
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
             const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
             const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL)
 {
+    constexpr int F = NUMA_DSS_FPT;
     const DssSeg sg = segs[blkmap[blockIdx.x]];
     const int t = (blockIdx.x - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
     if (t >= sg.n) return;
-    double *rm = r + (int64_t)threadIdx.y * NL;
+    double *rm = r + (int64_t)threadIdx.y * F * NL;
     if (sg.cls == 0) {
-        dss_node<2>(rm, idx + sg.idx_base, sg.n, t);
+        dss_node<2, F>(rm, idx + sg.idx_base, sg.n, t, NL);
     } else if (sg.cls == 1) {
-        dss_node<4>(rm, idx + sg.idx_base, sg.n, t);
+        dss_node<4, F>(rm, idx + sg.idx_base, sg.n, t, NL);
     } else if (sg.cls == 2) {
-        dss_node<8>(rm, idx + sg.idx_base, sg.n, t);
+        dss_node<8, F>(rm, idx + sg.idx_base, sg.n, t, NL);
     } else {
         const int gI = nodes[sg.node_off + t];
         const int s = start[gI], c = start[gI + 1] - s;
-        double sum = rm[copies[s]];
-        for (int a = 1; a < c; ++a) sum += rm[copies[s + a]];
-        for (int a = 0; a < c; ++a) rm[copies[s + a]] = sum;
+        for (int m = 0; m < F; ++m) {
+            double *rf = rm + (int64_t)m * NL;
+            double sum = rf[copies[s]];
+            for (int a = 1; a < c; ++a) sum += rf[copies[s + a]];
+            for (int a = 0; a < c; ++a) rf[copies[s + a]] = sum;
+        }
     }
 }
 
@@ -515,7 +539,7 @@ cudaError_t launch_dss_classes(numa_ctx *c, double *r, int kernel_id, cudaStream
 {
     if (c->dss_blocks == 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
-    k_stage_dss<<<(unsigned)c->dss_blocks, dim3(NUMA_DSS_THREADS, 5), 0, s>>>(
+    k_stage_dss<<<(unsigned)c->dss_blocks, dim3(NUMA_DSS_THREADS, 5 / NUMA_DSS_FPT), 0, s>>>(
         r, c->dss_idx, c->dss_seg, c->dss_blkmap, c->sh_nodes, c->dss_start, c->dss_copies, c->NL);
     return cudaGetLastError();
 }
