@@ -57,8 +57,18 @@ struct StageShape {
 #ifndef STAGE_NPT_MINN
 #define STAGE_NPT_MINN 9  /* measured: no gain at N <= 8; kept for larger elements */
 #endif
-    static constexpr int NPT = (N >= STAGE_NPT_MINN) ? STAGE_NPT_HI : 1;
-    static constexpr int THREADS = ((NODES + NPT - 1) / NPT + 31) / 32 * 32;
+    // THR_OVR: explicit block size where the default (one thread per node) balances the line
+    // tasks badly: 8*LINES tasks per direction should fill whole rounds of THREADS threads.
+#ifndef STAGE_THREADS5
+#define STAGE_THREADS5 0
+#endif
+#ifndef STAGE_THREADS6
+#define STAGE_THREADS6 416  /* 392 line tasks per pass in one round (352 threads: 352 + 40) */
+#endif
+    static constexpr int THR_OVR = (N == 5) ? STAGE_THREADS5 : (N == 6) ? STAGE_THREADS6 : 0;
+    static constexpr int NPT = THR_OVR ? (NODES + THR_OVR - 1) / THR_OVR
+                                       : (N >= STAGE_NPT_MINN) ? STAGE_NPT_HI : 1;
+    static constexpr int THREADS = THR_OVR ? THR_OVR : ((NODES + NPT - 1) / NPT + 31) / 32 * 32;
     static constexpr int SLOTS = THREADS * NPT;  // >= NODES
     static constexpr int LINES = EPB * N2;  // lines per field and direction
     // field stride in shared memory: = 2 (mod 4) doubles, so that with the FIELD-FASTEST task
@@ -79,7 +89,7 @@ struct StageShape {
 #ifndef STAGE_PREFETCH_MAXN
 #define STAGE_PREFETCH_MAXN 5
 #endif
-    static constexpr bool PREFETCH = (N <= STAGE_PREFETCH_MAXN);
+    static constexpr bool PREFETCH = (N <= STAGE_PREFETCH_MAXN) && NPT == 1;
     // PFS: the same 17 inputs are prefetched with cp.async into shared memory instead (no
     // registers held across phase B); used where one block per SM leaves the room (N = 6, 7).
 #ifndef STAGE_PFS_MASK
