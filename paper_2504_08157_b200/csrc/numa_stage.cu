@@ -36,7 +36,13 @@ struct StageShape {
 #ifndef STAGE_MINB4
 #define STAGE_MINB4 6
 #endif
-    static constexpr int EPB = (N == 2) ? 9 : (N == 3) ? 4 : (N == 4) ? STAGE_EPB4 : 1;
+#ifndef STAGE_EPB3
+#define STAGE_EPB3 2
+#endif
+#ifndef STAGE_EPB5
+#define STAGE_EPB5 1
+#endif
+    static constexpr int EPB = (N == 2) ? 9 : (N == 3) ? STAGE_EPB3 : (N == 4) ? STAGE_EPB4 : (N == 5) ? STAGE_EPB5 : 1;
     // shared node index i + SJ*j + SK*k; for even Nq the k-planes are padded by one double
     static constexpr int SJ = Nq;
     static constexpr int SK = (Nq & 1) ? N2 : N2 + 1;
@@ -99,7 +105,7 @@ struct StageShape {
     static constexpr int NPF = 17;  // met[9], omega, q0[5], heat, beta
     static constexpr size_t SMEM = SMEM_WORK + (PFS ? sizeof(double) * NPF * SLOTS : 0);
 #ifndef STAGE_MINB3
-#define STAGE_MINB3 3
+#define STAGE_MINB3 6
 #endif
 #ifndef STAGE_MINB5
 #define STAGE_MINB5 4
