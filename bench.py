@@ -277,9 +277,15 @@ def run_gpu(args):
         kb = kernel_alg_bytes(dom[0], mesh.N, has_src)
         achieved = kb * NL / (dom_ms / dom_n * 1e-3) / 1e9
         stage_ms = ms / (3 * args.steps)
+        # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+        # (profiles/r1c_fused_cfg3.md: dram__bytes_read.sum + dram__bytes_write.sum of a stage-1
+        # launch of k_stage_volume<4> on cfg3); other workloads have no capture -> null
+        traffic = 5.25e9 if (wl.name == "cfg3_tc_100x100x20_N4" and dom[0].startswith("k_stage_volume")) else None
         roofline = {
             "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": None, "kernel": dom[0],
+            "frac": achieved / peak, "traffic": traffic,
+            "traffic_source": "profiles/r1c_fused_cfg3.md (stage-1 launch: 200 algorithmic B/node = 5.00e9 B)" if traffic else None,
+            "kernel": dom[0],
             "kernel_ms": dom_ms / dom_n, "kernel_share_of_step": dom_ms / ms,
             "kernel_bytes_per_node": kb, "peak_source": peak_src,
             "stage": {"b_alg_bytes_per_node": balg, "ms": stage_ms,

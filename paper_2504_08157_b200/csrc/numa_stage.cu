@@ -85,10 +85,10 @@ struct StageShape {
     // POOLED: the zeta-derivatives get their own buffer, so the line tasks of all three
     // directions form one pool without a barrier in between (better balance at low N);
     // otherwise they overwrite the work fields in place after a barrier (less shared memory).
-#ifndef STAGE_POOLED_MAXN
-#define STAGE_POOLED_MAXN 2
+#ifndef STAGE_POOLED_MASK
+#define STAGE_POOLED_MASK 0x04  /* bit N set = pooled */
 #endif
-    static constexpr bool POOLED = (N <= STAGE_POOLED_MAXN);
+    static constexpr bool POOLED = (STAGE_POOLED_MASK >> N) & 1;
     static constexpr size_t SMEM_WORK = sizeof(double) * (POOLED ? 4 : 3) * NF * FS;
     // PREFETCH: request the phase-C inputs in phase A (17 doubles live across phase B); at high
     // N the registers are worth more as a second resident block.
