@@ -71,7 +71,10 @@ struct StageShape {
 #ifndef STAGE_THREADS6
 #define STAGE_THREADS6 416  /* 392 line tasks per pass in one round (352 threads: 352 + 40) */
 #endif
-    static constexpr int THR_OVR = (N == 5) ? STAGE_THREADS5 : (N == 6) ? STAGE_THREADS6 : 0;
+#ifndef STAGE_THREADS8
+#define STAGE_THREADS8 0
+#endif
+    static constexpr int THR_OVR = (N == 5) ? STAGE_THREADS5 : (N == 6) ? STAGE_THREADS6 : (N == 8) ? STAGE_THREADS8 : 0;
     static constexpr int NPT = THR_OVR ? (NODES + THR_OVR - 1) / THR_OVR
                                        : (N >= STAGE_NPT_MINN) ? STAGE_NPT_HI : 1;
     static constexpr int THREADS = THR_OVR ? THR_OVR : ((NODES + NPT - 1) / NPT + 31) / 32 * 32;
@@ -102,13 +105,16 @@ struct StageShape {
 #define STAGE_PFS_MASK 0x80  /* bit N set = use it (measured: pays at N = 7 only) */
 #endif
     static constexpr bool PFS = !PREFETCH && ((STAGE_PFS_MASK >> N) & 1);
-    static constexpr int NPF = 17;  // met[9], omega, q0[5], heat, beta
+    // PFS_ALL: all 17 inputs (met[9], omega, q0[5], heat, beta); otherwise only met and omega
+    // (N = 8: the other 7 do not fit beside the work buffers)
+    static constexpr bool PFS_ALL = (N != 8);
+    static constexpr int NPF = PFS_ALL ? 17 : 10;
     static constexpr size_t SMEM = SMEM_WORK + (PFS ? sizeof(double) * NPF * SLOTS : 0);
 #ifndef STAGE_MINB3
 #define STAGE_MINB3 6
 #endif
 #ifndef STAGE_MINB5
-#define STAGE_MINB5 4
+#define STAGE_MINB5 3
 #endif
 #ifndef STAGE_MINB6
 #define STAGE_MINB6 2
@@ -252,12 +258,14 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 #pragma unroll
             for (int c = 0; c < 9; ++c) cp_async8(d + c * SH::SLOTS, A.met + c * NL + p);
             cp_async8(d + 9 * SH::SLOTS, A.omega + p);
-            if (!same) {
+            if constexpr (SH::PFS_ALL) {
+                if (!same) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) cp_async8(d + (10 + c) * SH::SLOTS, A.q0 + c * NL + p);
+                    for (int c = 0; c < 5; ++c) cp_async8(d + (10 + c) * SH::SLOTS, A.q0 + c * NL + p);
+                }
+                if (A.heat) cp_async8(d + 15 * SH::SLOTS, A.heat + p);
+                if (A.beta) cp_async8(d + 16 * SH::SLOTS, A.beta + p);
             }
-            if (A.heat) cp_async8(d + 15 * SH::SLOTS, A.heat + p);
-            if (A.beta) cp_async8(d + 16 * SH::SLOTS, A.beta + p);
         }
 #pragma unroll
         for (int c = 0; c < 5; ++c) qv[rr][c] = A.qs[c * NL + p];
@@ -348,12 +356,21 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 #pragma unroll
         for (int c = 0; c < 9; ++c) m[c] = d[c * SH::SLOTS];
         om = d[9 * SH::SLOTS];
-        if (!same) {
+        if constexpr (SH::PFS_ALL) {
+            if (!same) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) q0v[c] = d[(10 + c) * SH::SLOTS];
+                for (int c = 0; c < 5; ++c) q0v[c] = d[(10 + c) * SH::SLOTS];
+            }
+            heat = A.heat ? d[15 * SH::SLOTS] : 0.0;
+            beta = A.beta ? d[16 * SH::SLOTS] : 0.0;
+        } else {
+            if (!same) {
+#pragma unroll
+                for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+            }
+            heat = A.heat ? __ldg(A.heat + p) : 0.0;
+            beta = A.beta ? __ldg(A.beta + p) : 0.0;
         }
-        heat = A.heat ? d[15 * SH::SLOTS] : 0.0;
-        beta = A.beta ? d[16 * SH::SLOTS] : 0.0;
     } else if constexpr (!SH::PREFETCH) {
 #pragma unroll
         for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
