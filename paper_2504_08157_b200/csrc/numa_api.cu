@@ -81,6 +81,13 @@ void numa_build_lgl(int N, LglTables *t)
         }
         t->D[i * Nq + i] = (double)diag;
     }
+    // exact centro-antisymmetry D[N-i][N-l] = -D[i][l] (the kernels use only the upper half)
+    for (int i = 0; i < Nq; ++i)
+        for (int l = 0; l < Nq; ++l) {
+            const int a = i * Nq + l, b = (N - i) * Nq + (N - l);
+            if (a < b) t->D[b] = -t->D[a];
+            else if (a == b) t->D[a] = 0.0;
+        }
 }
 
 // ---------------------------------------------------------------------------------------

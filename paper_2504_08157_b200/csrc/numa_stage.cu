@@ -102,7 +102,7 @@ struct StageShape {
     // PFS: the same 17 inputs are prefetched with cp.async into shared memory instead (no
     // registers held across phase B); used where one block per SM leaves the room (N = 6, 7).
 #ifndef STAGE_PFS_MASK
-#define STAGE_PFS_MASK 0x80  /* bit N set = use it (measured: pays at N = 7 only) */
+#define STAGE_PFS_MASK 0x100  /* bit N set = use it (measured: pays at N = 8 only) */
 #endif
     static constexpr bool PFS = !PREFETCH && ((STAGE_PFS_MASK >> N) & 1);
     // PFS_ALL: all 17 inputs (met[9], omega, q0[5], heat, beta); otherwise only met and omega
@@ -120,7 +120,7 @@ struct StageShape {
 #define STAGE_MINB6 2
 #endif
 #ifndef STAGE_MINB7
-#define STAGE_MINB7 1
+#define STAGE_MINB7 2
 #endif
 #ifndef STAGE_MINB8
 #define STAGE_MINB8 1
@@ -154,6 +154,11 @@ __device__ __forceinline__ double eos_ratio(double x, double gamma, const double
     return expm1(gamma * log1p(x));
 }
 
+// All Nq derivatives of one line.  D is centro-antisymmetric (D[N-m][N-l] = -D[m][l], enforced
+// bitwise by numa_build_lgl), so rows m and N-m share their constants: only the upper half of
+// D is touched -- on sm_100 constant operands travel through uniform registers, and the full
+// (N+1)^2 table does not fit them at N >= 6 (the compiler then spills through vector registers
+// to local memory).
 template <int Nq>
 __device__ __forceinline__ void line_derivs(const double *src, int sstride, double *dst,
                                             const LglTables &tab)
@@ -161,12 +166,37 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
     double x[Nq];
 #pragma unroll
     for (int l = 0; l < Nq; ++l) x[l] = src[sstride * l];
+#ifndef STAGE_ANTISYM_MINNQ
+#define STAGE_ANTISYM_MINNQ 7  /* N >= 6; below that the full table fits and is faster */
+#endif
+    if constexpr (Nq < STAGE_ANTISYM_MINNQ) {
 #pragma unroll
-    for (int m = 0; m < Nq; ++m) {
-        double acc = 0.0;
+        for (int m = 0; m < Nq; ++m) {
+            double acc = 0.0;
 #pragma unroll
-        for (int l = 0; l < Nq; ++l) acc = fma(tab.D[m * Nq + l], x[l], acc);
-        dst[sstride * m] = acc;
+            for (int l = 0; l < Nq; ++l) acc = fma(tab.D[m * Nq + l], x[l], acc);
+            dst[sstride * m] = acc;
+        }
+        return;
+    }
+#pragma unroll
+    for (int m = 0; m < Nq / 2; ++m) {
+        double a = 0.0, b = 0.0;
+#pragma unroll
+        for (int l = 0; l < Nq; ++l) {
+            const double d = tab.D[m * Nq + l];
+            a = fma(d, x[l], a);
+            b = fma(d, x[Nq - 1 - l], b);
+        }
+        dst[sstride * m] = a;
+        dst[sstride * (Nq - 1 - m)] = -b;
+    }
+    if constexpr (Nq & 1) {
+        constexpr int m = Nq / 2;
+        double a = 0.0;
+#pragma unroll
+        for (int l = 0; l < Nq; ++l) a = fma(tab.D[m * Nq + l], x[l], a);
+        dst[sstride * m] = a;
     }
 }
 
@@ -329,6 +359,9 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
             const int base = f * FS + el * ME;
             const int bx = base + ((Nq & 1) ? SJ * lo + SK * hi : SJ * hi + SK * lo);
             line_derivs<Nq>(sW + bx, 1, sGx + bx, tab);
+#ifdef STAGE_SPLIT_XY
+            if constexpr (N >= STAGE_SPLIT_XY) asm volatile("" ::: "memory");  // keep the two lines' registers apart
+#endif
             line_derivs<Nq>(sW + base + lo + SK * hi, SJ, sGe + base + lo + SK * hi, tab);
         }
         __syncthreads();
