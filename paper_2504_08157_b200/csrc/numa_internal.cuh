@@ -19,7 +19,9 @@ struct LglTables {
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
 enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_COUNT = 6 };
 
-#define NUMA_DSS_CHUNK 32768   // local nodes per DSS locality chunk
+#ifndef NUMA_DSS_CHUNK
+#define NUMA_DSS_CHUNK 2048    // local nodes per DSS locality chunk (measured best of 256..2 M on cfg3)
+#endif
 #ifndef NUMA_DSS_THREADS
 #define NUMA_DSS_THREADS 64    // shared nodes per thread block of the DSS kernel
 #endif

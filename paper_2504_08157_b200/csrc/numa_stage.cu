@@ -177,26 +177,26 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
             for (int l = 0; l < Nq; ++l) acc = fma(tab.D[m * Nq + l], x[l], acc);
             dst[sstride * m] = acc;
         }
-        return;
-    }
+    } else {
 #pragma unroll
-    for (int m = 0; m < Nq / 2; ++m) {
-        double a = 0.0, b = 0.0;
+        for (int m = 0; m < Nq / 2; ++m) {
+            double a = 0.0, b = 0.0;
 #pragma unroll
-        for (int l = 0; l < Nq; ++l) {
-            const double d = tab.D[m * Nq + l];
-            a = fma(d, x[l], a);
-            b = fma(d, x[Nq - 1 - l], b);
+            for (int l = 0; l < Nq; ++l) {
+                const double d = tab.D[m * Nq + l];
+                a = fma(d, x[l], a);
+                b = fma(d, x[Nq - 1 - l], b);
+            }
+            dst[sstride * m] = a;
+            dst[sstride * (Nq - 1 - m)] = -b;
         }
-        dst[sstride * m] = a;
-        dst[sstride * (Nq - 1 - m)] = -b;
-    }
-    if constexpr (Nq & 1) {
-        constexpr int m = Nq / 2;
-        double a = 0.0;
+        if constexpr (Nq & 1) {
+            constexpr int m = Nq / 2;
+            double a = 0.0;
 #pragma unroll
-        for (int l = 0; l < Nq; ++l) a = fma(tab.D[m * Nq + l], x[l], a);
-        dst[sstride * m] = a;
+            for (int l = 0; l < Nq; ++l) a = fma(tab.D[m * Nq + l], x[l], a);
+            dst[sstride * m] = a;
+        }
     }
 }
 
