@@ -74,7 +74,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "25"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -83,9 +83,11 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append(line.strip())
+            self.rows.append((time.time(), line.strip()))
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """Median SM clock and throttle reasons of the samples that arrived in [t0, t1] (wall
+        clock of the timed region; all samples if none fell inside)."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
@@ -96,7 +98,10 @@ class ClockSampler:
             self.proc.kill()
         sm, smax, reasons = [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        rows = [r for (t, r) in self.rows if t0 is None or (t0 <= t <= (t1 or t) + 0.03)]
+        if not rows:
+            rows = [r for (t, r) in self.rows if t0 is None or t >= t0] or [r for (_, r) in self.rows]
+        for r in rows:
             parts = [p.strip() for p in r.split(",")]
             if len(parts) < 7:
                 continue
@@ -223,19 +228,29 @@ def run_gpu(args):
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
+        time.sleep(0.3)   # nvidia-smi needs a moment before its first sample; untimed
     g.profile(True)
     l0 = g.launch_count
     ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
     barrier()
+    wall0 = time.time()
     ev0.record(stream)
     g.step_rk3(q, wl.dt, heat, args.steps)
     ev1.record(stream)
     barrier()
+    wall1 = time.time()
     ms = ev0.elapsed_time(ev1)
     launches = g.launch_count - l0
     prof = g.profile_read()
     g.profile(False)
-    clocks = sampler.stop() if rank == 0 else None
+    if rank == 0 and not any(wall0 <= t <= wall1 + 0.03 for (t, _) in sampler.rows):
+        # very short timed region: keep the same load running until a sample has been taken
+        n0 = len(sampler.rows)
+        t_end = time.time() + 3.0
+        while len(sampler.rows) == n0 and time.time() < t_end:
+            g.step_rk3(q, wl.dt, heat, 5)
+            torch.cuda.synchronize()
+    clocks = sampler.stop(wall0, wall1) if rank == 0 else None
     finite = bool(torch.isfinite(q).all().item())
     ms = max_over_ranks(ms, dev, world)
 
@@ -278,13 +293,13 @@ def run_gpu(args):
         achieved = kb * NL / (dom_ms / dom_n * 1e-3) / 1e9
         stage_ms = ms / (3 * args.steps)
         # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-        # (profiles/r1c_fused_cfg3.md: dram__bytes_read.sum + dram__bytes_write.sum of a stage-1
+        # (profiles/r1e_final_cfg3.md: dram__bytes_read.sum + dram__bytes_write.sum of a stage-1
         # launch of k_stage_volume<4> on cfg3); other workloads have no capture -> null
         traffic = 5.25e9 if (wl.name == "cfg3_tc_100x100x20_N4" and dom[0].startswith("k_stage_volume")) else None
         roofline = {
             "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
             "frac": achieved / peak, "traffic": traffic,
-            "traffic_source": "profiles/r1c_fused_cfg3.md (stage-1 launch: 200 algorithmic B/node = 5.00e9 B)" if traffic else None,
+            "traffic_source": "profiles/r1e_final_cfg3.md (stage-1 launch: 200 algorithmic B/node = 5.00e9 B)" if traffic else None,
             "kernel": dom[0],
             "kernel_ms": dom_ms / dom_n, "kernel_share_of_step": dom_ms / ms,
             "kernel_bytes_per_node": kb, "peak_source": peak_src,
@@ -349,7 +364,7 @@ def kernel_alg_bytes(name, N, has_src):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="numa_b200", choices=["numa_b200", "reference"])
     ap.add_argument("--workload", default="cfg3")
