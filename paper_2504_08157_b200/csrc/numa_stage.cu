@@ -523,7 +523,10 @@ __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__
 }
 
 // block = (NUMA_DSS_THREADS shared nodes) x (5 / NUMA_DSS_FPT field groups)
-__global__ void __launch_bounds__(NUMA_DSS_THREADS * (5 / NUMA_DSS_FPT))
+#ifndef NUMA_DSS_MINB
+#define NUMA_DSS_MINB 1
+#endif
+__global__ void __launch_bounds__(NUMA_DSS_THREADS * (5 / NUMA_DSS_FPT), NUMA_DSS_MINB)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
             const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
             const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL)
