@@ -81,6 +81,23 @@ void numa_build_lgl(int N, LglTables *t)
         }
         t->D[i * Nq + i] = (double)diag;
     }
+    {   // even-odd split, from the long double values
+        const int H = Nq / 2;
+        for (int k = 0; k < 16; ++k) t->A[k] = t->B[k] = 0.0;
+        for (int k = 0; k < 4; ++k) t->C[k] = t->M[k] = 0.0;
+        auto Dld = [&](int i, int l) -> long double {
+            if (i == l) { long double d = 0.0L; for (int k = 0; k < Nq; ++k) if (k != i) d -= (bw[k] / bw[i]) / (x[i] - x[k]); return d; }
+            return (bw[l] / bw[i]) / (x[i] - x[l]);
+        };
+        for (int m = 0; m < H; ++m) {
+            for (int l = 0; l < H; ++l) {
+                t->A[m * H + l] = (double)(0.5L * (Dld(m, l) + Dld(m, N - l)));
+                t->B[m * H + l] = (double)(0.5L * (Dld(m, l) - Dld(m, N - l)));
+            }
+            if (Nq & 1) t->C[m] = (double)Dld(m, H);
+        }
+        if (Nq & 1) for (int l = 0; l < H; ++l) t->M[l] = (double)Dld(H, l);
+    }
     // exact centro-antisymmetry D[N-i][N-l] = -D[i][l] (the kernels use only the upper half)
     for (int i = 0; i < Nq; ++i)
         for (int l = 0; l < Nq; ++l) {

@@ -14,6 +14,9 @@
 struct LglTables {
     double D[NUMA_MAX_NQ * NUMA_MAX_NQ];  // D[i*Nq + l] = h_l'(xi_i)  (Alg. 2)
     double w[NUMA_MAX_NQ];                // quadrature weights (Eq. 8)
+    // even-odd split of D (H = Nq/2): A[m*H+l] = (D[m][l] + D[m][N-l])/2, B = (D[m][l] - D[m][N-l])/2,
+    // C[m] = D[m][H] and M[l] = D[H][l] (odd Nq only); used by the line contraction at N >= 6
+    double A[16], B[16], C[4], M[4];
 };
 
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)

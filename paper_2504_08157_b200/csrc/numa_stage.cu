@@ -177,6 +177,31 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
             for (int l = 0; l < Nq; ++l) acc = fma(tab.D[m * Nq + l], x[l], acc);
             dst[sstride * m] = acc;
         }
+#ifndef STAGE_EVEN_ODD
+#define STAGE_EVEN_ODD 7  /* Nq from which the even-odd form is used (measured: pays at N >= 6) */
+#endif
+#if STAGE_EVEN_ODD > 0
+    } else if constexpr (Nq >= STAGE_EVEN_ODD) {
+        // even-odd form: half the multiplications (A, B of LglTables)
+        constexpr int H = Nq / 2;
+        double e[H], o[H];
+#pragma unroll
+        for (int l = 0; l < H; ++l) { e[l] = x[l] + x[Nq - 1 - l]; o[l] = x[l] - x[Nq - 1 - l]; }
+#pragma unroll
+        for (int m = 0; m < H; ++m) {
+            double P = (Nq & 1) ? tab.C[m] * x[H] : 0.0, Q = 0.0;
+#pragma unroll
+            for (int l = 0; l < H; ++l) { P = fma(tab.A[m * H + l], e[l], P); Q = fma(tab.B[m * H + l], o[l], Q); }
+            dst[sstride * m] = P + Q;
+            dst[sstride * (Nq - 1 - m)] = Q - P;
+        }
+        if constexpr (Nq & 1) {
+            double a = 0.0;
+#pragma unroll
+            for (int l = 0; l < H; ++l) a = fma(tab.M[l], o[l], a);
+            dst[sstride * H] = a;
+        }
+#endif
     } else {
 #pragma unroll
         for (int m = 0; m < Nq / 2; ++m) {
@@ -524,7 +549,7 @@ __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__
 
 // block = (NUMA_DSS_THREADS shared nodes) x (5 / NUMA_DSS_FPT field groups)
 #ifndef NUMA_DSS_MINB
-#define NUMA_DSS_MINB 1
+#define NUMA_DSS_MINB 10  /* 96 registers; measured: neither more (12-20) nor fewer (1) resident blocks is faster */
 #endif
 __global__ void __launch_bounds__(NUMA_DSS_THREADS * (5 / NUMA_DSS_FPT), NUMA_DSS_MINB)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
