@@ -21,8 +21,10 @@
  *   (>= 8-byte aligned; 16-byte alignment enables the vectorised paths) and stays
  *   caller-owned.  The library allocates no device memory: persistent tables live in the
  *   caller-provided workspace handed to numa_init_geometry.  `stream` is a cudaStream_t
- *   passed as void* (NULL = legacy default stream).  All calls except numa_init_geometry
- *   and the *_host calls only enqueue work on `stream` and return without synchronising.
+ *   passed as void* (NULL = legacy default stream).  All calls except numa_init_geometry,
+ *   the *_host calls and numa_copy_table(which >= 3) only enqueue work on `stream` and return
+ *   without synchronising.  A context belongs to the device that was current when
+ *   numa_init_geometry created it; calling it with another device current is NUMA_ERR_ARG.
  *
  * Errors
  *   Every call returns a numa_status; nothing throws.  Argument checks are synchronous and
@@ -68,7 +70,8 @@ typedef struct {
 /* Bytes of device workspace numa_init_geometry needs for these parameters (0 on bad input). */
 size_t numa_workspace_bytes(const numa_params *p);
 
-/* Bytes of device scratch numa_step_rk3 needs (one state-sized buffer: the stage state). */
+/* Bytes of device scratch numa_step_rk3 needs (two state-sized buffers in the block-shell
+ * layout: the state of the step and the stage state). */
 size_t numa_step_scratch_bytes(const numa_params *p);
 
 /*
@@ -129,13 +132,42 @@ numa_status numa_rk_stage(numa_ctx *ctx, double a0, double a1, double b_dt, cons
                           const double *qs, const double *rhs, double *q_out, void *stream);
 
 /*
- * A11 -- n_steps SSP-RK3 (Shu-Osher) steps of size dt, in place on q[5][Ne][Mn], through the
- * fused kernels (same mathematics as numa_rhs -> numa_dss_or_flux -> numa_apply_sources ->
- * numa_rk_stage per stage; both routes are parity-tested).  heating may be NULL.
- * scratch: >= numa_step_scratch_bytes(p) bytes, 256-byte aligned.
+ * A11 -- n_steps SSP-RK3 (Shu-Osher, Q11) steps of size dt, in place on
+ * q[5][Ne][Mn], through the FUSED stage (two kernels per stage instead of four):
+ *   q_out = a0*q0 + a1*qs + b_dt*L(qs),  L = walls(sources(DSS(omega*S)))  as defined by the
+ * four calls above.  The volume kernel writes omega*(a0 q0 + a1 qs) + b_dt*P(omega*(S + src))
+ * -- the stage update as DSS partial sums -- and the DSS kernel completes the shared nodes in
+ * place; equal to the four-call route up to rounding because DSS is linear and
+ * sum_copies(omega) = 1.  Both routes are parity-tested.
+ * PRECONDITIONS of that identity (the four-call route needs none of them):
+ *   (1) q, heating and sponge are single-valued at a global node: all local copies of a node
+ *       hold bitwise the same value (true for any state this library produced and for nodal
+ *       data sampled once per global node);
+ *   (2) the no-flux projector is the same in every element sharing a wall node, i.e. the
+ *       walls are planar (or the metric-derived normals agree across the copies);
+ *   (3) every element that touches a wall node owns a wall face at that node.
+ * Box meshes with planar walls (all BASELINE.json configurations) satisfy all three.  Where
+ * (2) or (3) fails the fused route averages the projected tendencies of the copies with the
+ * weights omega instead of projecting the assembled tendency: use the four-call route there.
+ *
+ * Inside the call the state is kept in a block-shell layout in `scratch`; q is
+ * converted on entry and written back (natural layout) before the call returns, so the cost
+ * of the two conversions is amortised over n_steps.
+ * heating may be NULL; it is held constant over the n_steps (the caller refreshes it between
+ * calls: BASELINE.json config 3 "refreshed every 60 s").
+ * scratch: >= numa_step_scratch_bytes(p) bytes (two states), 256-byte aligned.
+ *
+ * numa_step_rk3_graph: the same steps with the three stages of a step captured once into a
+ * CUDA graph (cached in the context, keyed by the pointer arguments, dt and stream) and
+ * replayed n_steps times -- same kernels, same results bit for bit, one launch call per step
+ * instead of six; meant for meshes so small that a stage is shorter than its launch overhead
+ * (BASELINE.json configs 1-2).  Falls back to plain launches when `stream`
+ * is itself being captured by the caller.
  */
 numa_status numa_step_rk3(numa_ctx *ctx, double *q, void *scratch, const double *heating,
                           double dt, int32_t n_steps, void *stream);
+numa_status numa_step_rk3_graph(numa_ctx *ctx, double *q, void *scratch, const double *heating,
+                                double dt, int32_t n_steps, void *stream);
 
 /*
  * End-to-end variant with HOST buffers: copies q (and heating, if non-NULL) host -> device
@@ -154,21 +186,6 @@ numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heat
  * 3a+c), 1 omega[NL], 2 p0[NL], 3 D[Nq*Nq] (D[i*Nq+l] = h_l'(xi_i)), 4 w[Nq].
  */
 numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, double *out, void *stream);
-
-/*
- * Optional per-kernel timing with CUDA events recorded on the launching stream around every
- * kernel this context launches (bench.py's roofline figure).  numa_profile_enable(ctx, 1)
- * clears the accumulators and starts recording, (ctx, 0) stops.  numa_profile_read waits for
- * the recorded events and returns the accumulated device time and launch count of one
- * kernel id: 0 volume (numa_rhs), 1 DSS, 2 sources, 3 RK stage, 4 fused stage volume,
- * 5 fused stage DSS.  numa_kernel_name gives a printable name.
- */
-numa_status numa_profile_enable(numa_ctx *ctx, int32_t enable);
-numa_status numa_profile_read(numa_ctx *ctx, int32_t kernel_id, double *total_ms, int64_t *launches);
-const char *numa_kernel_name(int32_t kernel_id);
-
-/* Number of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
-int64_t numa_launch_count(const numa_ctx *ctx);
 
 numa_status numa_destroy(numa_ctx *ctx);
 

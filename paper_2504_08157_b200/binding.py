@@ -18,10 +18,13 @@ _LIB = None
 STATUS = {0: "NUMA_OK", 1: "NUMA_ERR_ARG", 2: "NUMA_ERR_UNSUPPORTED", 3: "NUMA_ERR_CUDA",
           4: "NUMA_ERR_NEG_JACOBIAN", 5: "NUMA_ERR_WORKSPACE"}
 
+# product ABI (include/numa_b200.h) and measurement ABI (include/numa_b200_measure.h)
 EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometry", "numa_rhs",
            "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
-           "numa_step_rk3_host", "numa_copy_table", "numa_launch_count", "numa_destroy",
-           "numa_last_error", "numa_profile_enable", "numa_profile_read", "numa_kernel_name"]
+           "numa_step_rk3_graph", "numa_step_rk3_host", "numa_copy_table", "numa_destroy",
+           "numa_last_error"]
+MEASURE_EXPORTS = ["numa_profile_enable", "numa_profile_read", "numa_kernel_name",
+                   "numa_kernel_count", "numa_launch_count", "numa_measure_fp64_peak"]
 
 
 class NumaParams(C.Structure):
@@ -42,8 +45,9 @@ def load_library(path: str | None = None):
     global _LIB
     if _LIB is not None and path is None:
         return _LIB
-    libpath = path or _build.LIB
-    if path is None and (not os.path.exists(libpath) or os.environ.get("NUMA_B200_REBUILD")):
+    # NUMA_B200_LIB: development knob to load a differently tuned build of the library
+    libpath = path or os.environ.get("NUMA_B200_LIB") or _build.LIB
+    if path is None and not os.environ.get("NUMA_B200_LIB") and (not os.path.exists(libpath) or os.environ.get("NUMA_B200_REBUILD")):
         libpath = _build.build()
     if not os.path.exists(libpath):
         raise ImportError("libnuma_b200.so is missing and could not be built; there is no "
@@ -61,6 +65,7 @@ def load_library(path: str | None = None):
     L.numa_apply_sources.argtypes = [vp, dp, dp, dp, vp]
     L.numa_rk_stage.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp, vp]
     L.numa_step_rk3.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
+    L.numa_step_rk3_graph.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
     L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
     L.numa_profile_enable.argtypes = [vp, C.c_int32]
@@ -69,13 +74,18 @@ def load_library(path: str | None = None):
     L.numa_profile_read.restype = C.c_int
     L.numa_kernel_name.argtypes = [C.c_int32]
     L.numa_kernel_name.restype = C.c_char_p
+    L.numa_kernel_count.argtypes = []
+    L.numa_kernel_count.restype = C.c_int32
+    L.numa_measure_fp64_peak.argtypes = [C.c_int32, C.POINTER(C.c_double), vp]
+    L.numa_measure_fp64_peak.restype = C.c_int
     L.numa_launch_count.argtypes = [vp]
     L.numa_launch_count.restype = C.c_int64
     L.numa_destroy.argtypes = [vp]
     L.numa_last_error.argtypes = [vp]
     L.numa_last_error.restype = C.c_char_p
     for f in ("numa_init_geometry", "numa_rhs", "numa_dss_or_flux", "numa_apply_sources",
-              "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_host", "numa_copy_table",
+              "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_graph", "numa_step_rk3_host",
+              "numa_copy_table",
               "numa_destroy"):
         getattr(L, f).restype = C.c_int
     if path is None:
@@ -190,9 +200,9 @@ class Numa:
                                            _ptr(out), _stream()))
         return out
 
-    def step_rk3(self, q, dt, heating=None, n_steps=1):
-        self._check(self.lib.numa_step_rk3(self.ctx, _ptr(q), _ptr(self.scratch()), _ptr(heating),
-                                           dt, n_steps, _stream()))
+    def step_rk3(self, q, dt, heating=None, n_steps=1, graph=False):
+        fn = self.lib.numa_step_rk3_graph if graph else self.lib.numa_step_rk3
+        self._check(fn(self.ctx, _ptr(q), _ptr(self.scratch()), _ptr(heating), dt, n_steps, _stream()))
         return q
 
     def step_rk3_host(self, q_host, dt, heating_host=None, n_steps=1, d_q=None, d_heating=None):
@@ -219,12 +229,20 @@ class Numa:
     def profile_read(self):
         """{kernel name: (total device ms, launches)} accumulated since profile(True)."""
         out = {}
-        for kid in range(6):
+        for kid in range(self.lib.numa_kernel_count()):
             ms = C.c_double(); n = C.c_int64()
             self._check(self.lib.numa_profile_read(self.ctx, kid, C.byref(ms), C.byref(n)))
             if n.value:
                 out[self.lib.numa_kernel_name(kid).decode()] = (ms.value, n.value)
         return out
+
+    def fp64_peak_tflops(self, repeats=5):
+        """Measured DFMA ceiling of the current device (numa_measure_fp64_peak)."""
+        v = C.c_double()
+        st = self.lib.numa_measure_fp64_peak(repeats, C.byref(v), _stream())
+        if st != 0:
+            raise NumaError(st, "numa_measure_fp64_peak")
+        return v.value
 
     @property
     def launch_count(self):

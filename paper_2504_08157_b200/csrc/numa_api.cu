@@ -5,6 +5,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
 
 #include "numa_internal.cuh"
@@ -113,40 +115,67 @@ void numa_build_lgl(int N, LglTables *t)
 static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 static const size_t kSmallTmp = (size_t)4 << 20;  // CUB temp storage for small meshes
+static const size_t kSmallScr = (size_t)2 << 20;  // list-building scratch for meshes too small to lend their `met` region
+
+struct DssOff { size_t start, copies, sh_nodes, idx, seg, blkmap; };
 
 struct WsLayout {
-    size_t met, omega, ref3, sponge, start, copies, sh_nodes, dss_idx, dss_seg, dss_blkmap, face_bc, flags, small_tmp, total;
-    size_t scratch_bytes;  // init-time scratch, aliased onto the (not yet written) met region
+    size_t met, omega, ref3, sponge, face_bc, flags, small_tmp, shell_pos, shell_inv, shell_tab, total;
+    DssOff nat, shl;
+    ShellLayout shell;  // sizes only (pos = nullptr)
 };
 
-static inline size_t WsMaxSeg(size_t NL) { return 4 * (NL / NUMA_DSS_CHUNK + 2); }
+static inline size_t WsMaxSeg(size_t n_pos) { return 4 * (n_pos / NUMA_DSS_CHUNK + 2); }
 
 static bool params_ok(const numa_params *p)
 {
     return p && p->N >= 2 && p->N <= 8 && p->n_elem > 0 && p->n_global > 0 &&
-           p->n_elem * (int64_t)((p->N + 1) * (p->N + 1) * (p->N + 1)) < (int64_t)2147483647 &&
+           p->n_elem * (int64_t)((p->N + 1) * (p->N + 1) * (p->N + 1)) < (int64_t)2147483647 - 65536 &&
            p->n_global < (int64_t)2147483647 && p->c_v > 0 && p->c_p > 0 && p->p_a > 0 && p->R_gas > 0;
+}
+
+static ShellLayout shell_sizes(const numa_params *p)
+{
+    ShellLayout sh;
+    const int64_t Nq = p->N + 1, Mn = Nq * Nq * Nq;
+    sh.epb = stage_epb(p->N);
+    sh.BS = (sh.epb * Mn + 31) / 32 * 32;   // whole warps: every block record starts on a 256-byte line
+    sh.n_blocks = (p->n_elem + sh.epb - 1) / sh.epb;
+    sh.FS = sh.n_blocks * sh.BS;
+    return sh;
+}
+
+static size_t dss_layout(DssOff &d, size_t off, size_t n_pos, size_t NG)
+{
+    const size_t max_seg = WsMaxSeg(n_pos);
+    d.start = off; off = align_up(off + (NG + 1) * 4);
+    d.copies = off; off = align_up(off + n_pos * 4);
+    d.sh_nodes = off; off = align_up(off + (NG + 1) * 4);
+    d.idx = off; off = align_up(off + n_pos * 4);
+    d.seg = off; off = align_up(off + max_seg * sizeof(DssSeg));
+    d.blkmap = off; off = align_up(off + (NG / NUMA_DSS_THREADS + max_seg + 1) * 4);
+    return off;
 }
 
 static WsLayout ws_layout(const numa_params *p)
 {
     WsLayout L;
     const size_t Nq = p->N + 1, Mn = Nq * Nq * Nq, NL = (size_t)p->n_elem * Mn;
+    L.shell = shell_sizes(p);
     size_t off = 0;
-    L.met = off; off = align_up(off + 9 * NL * 8);
-    L.omega = off; off = align_up(off + NL * 8);
-    L.ref3 = off; off = align_up(off + 3 * NL * 8);
-    L.sponge = off; off = align_up(off + NL * 8);
-    L.start = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
-    L.copies = off; off = align_up(off + NL * 4);
-    L.sh_nodes = off; off = align_up(off + ((size_t)p->n_global + 1) * 4);
-    L.dss_idx = off; off = align_up(off + NL * 4);
-    const size_t max_seg = WsMaxSeg(NL);
-    L.dss_seg = off; off = align_up(off + max_seg * sizeof(DssSeg));
-    L.dss_blkmap = off; off = align_up(off + ((size_t)p->n_global / NUMA_DSS_THREADS + max_seg + 1) * 4);
+    const size_t FS = (size_t)L.shell.FS;   // the tables are block-shell arrays
+    L.met = off; off = align_up(off + 9 * FS * 8);
+    L.omega = off; off = align_up(off + FS * 8);
+    L.ref3 = off; off = align_up(off + 3 * FS * 8);
+    L.sponge = off; off = align_up(off + FS * 8);
+    off = dss_layout(L.nat, off, NL, (size_t)p->n_global);
+    off = dss_layout(L.shl, off, (size_t)L.shell.FS, (size_t)p->n_global);
+    L.shell_pos = off; off = align_up(off + (size_t)L.shell.epb * Mn * 4);
+    L.shell_inv = off; off = align_up(off + (size_t)L.shell.BS * 4);
+    L.shell_tab = off; off = align_up(off + (size_t)L.shell.BS * 4);
     L.face_bc = off; off = align_up(off + (size_t)p->n_elem * 8);
     L.flags = off; off = align_up(off + 256);
-    L.small_tmp = off; off = align_up(off + kSmallTmp);
+    L.small_tmp = off; off = align_up(off + kSmallTmp + kSmallScr);
     L.total = off;
     return L;
 }
@@ -157,29 +186,74 @@ extern "C" size_t numa_workspace_bytes(const numa_params *p)
     return ws_layout(p).total;
 }
 
+// block-shell scratch of numa_step_rk3: the state of the step, the stage state, the heating
+static inline size_t shell_state_bytes(const ShellLayout &sh) { return align_up((size_t)5 * sh.FS * 8); }
+static inline size_t shell_field_bytes(const ShellLayout &sh) { return align_up((size_t)sh.FS * 8); }
+
 extern "C" size_t numa_step_scratch_bytes(const numa_params *p)
 {
     if (!params_ok(p)) return 0;
-    const size_t Nq = p->N + 1, NL = (size_t)p->n_elem * Nq * Nq * Nq;
-    return align_up(5 * NL * 8);
+    const ShellLayout sh = shell_sizes(p);
+    return 2 * shell_state_bytes(sh) + shell_field_bytes(sh);
+}
+
+// the layout tables depend on (N, epb) only: built once per process
+struct ShellTables { std::vector<int32_t> pos; std::vector<uint32_t> tab; };
+static const ShellTables &shell_tables(int N, int epb, int64_t BS)
+{
+    static std::mutex mu;
+    static std::map<std::pair<int, int>, ShellTables> cache;
+    std::lock_guard<std::mutex> lock(mu);
+    auto key = std::make_pair(N, epb);
+    auto it = cache.find(key);
+    if (it == cache.end()) {
+        ShellTables t;
+        numa_build_shell_pos(N, epb, BS, t.pos, t.tab);
+        it = cache.emplace(key, std::move(t)).first;
+    }
+    return it->second;
 }
 
 // ---------------------------------------------------------------------------------------
 // setup kernels
 // ---------------------------------------------------------------------------------------
-__global__ void k_iota_check(int32_t *vals, const int32_t *keys_in, int32_t *keys, int64_t n,
-                             int64_t NG, int32_t *flags)
+// every intma_cg entry must lie in [0, NG): checked BEFORE anything is indexed with it
+__global__ void k_check_ids(const int32_t *__restrict__ cg, int64_t n, int64_t NG, int32_t *flags)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    int bad = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const int32_t g = keys_in[i];
-        if (g < 0 || g >= NG) atomicOr(flags + 1, 1);
-        keys[i] = g;
-        vals[i] = (int32_t)i;
+        const int32_t g = cg[i];
+        bad |= (g < 0 || g >= NG);
+    }
+    if (bad) atomicOr(flags + 1, 1);
+}
+
+// sort input of one list set: position t of the index space -> (key = global id, value = t).
+// Natural order: t = local node.  Block-shell order: t = b*BS + r, r -> (le, n) through the
+// inverse table; holes of the layout (padding, elements past Ne) get the sentinel key NG.
+__global__ void k_sort_input(int32_t *__restrict__ vals, int32_t *__restrict__ keys,
+                             const int32_t *__restrict__ cg, int64_t n_pos, int64_t NG,
+                             const int32_t *__restrict__ inv, int64_t BS, int epb, int64_t Mn,
+                             int64_t Ne)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n_pos; t += stride) {
+        int32_t key;
+        if (inv == nullptr) key = cg[t];
+        else {
+            const int64_t b = t / BS, r = t - b * BS;
+            const int32_t ln = inv[r];  // le*Mn + n, or -1
+            const int64_t e = b * epb + (ln >= 0 ? ln / Mn : 0);
+            key = (ln >= 0 && e < Ne) ? cg[e * Mn + (ln % Mn)] : (int32_t)NG;
+        }
+        keys[t] = key;
+        vals[t] = (int32_t)t;
     }
 }
 
-// start[g] = first position in the sorted key array whose key is >= g
+// start[g] = first position in the sorted key array whose key is >= g, g = 0..NG
+// (keys are in [0, NG]; NG is the sentinel of layout holes and sorts last)
 __global__ void k_find_starts(const int32_t *__restrict__ keys, int32_t *__restrict__ start,
                               int64_t n, int64_t NG)
 {
@@ -244,15 +318,19 @@ k_class_lists(const int32_t *__restrict__ nodes, const int32_t *__restrict__ sta
     for (int a = 0; a < C; ++a) idx[sg.idx_base + (int64_t)a * sg.n + t] = copies[s + a];
 }
 
+// ref (natural) -> ref3 (block-shell): rho0, theta0, p0
 __global__ void k_ref3(const double *__restrict__ ref, double *__restrict__ ref3, int64_t NL,
-                       double p_a, double R, double gamma)
+                       double p_a, double R, double gamma, const int32_t *__restrict__ pos, int npb,
+                       int BS, int64_t FS)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; p < NL; p += stride) {
+        const int64_t b = p / npb;
+        const int64_t t = b * BS + pos[p - b * npb];
         const double rho0 = ref[p], th0 = ref[NL + p];
-        ref3[p] = rho0;
-        ref3[NL + p] = th0;
-        ref3[2 * NL + p] = p_a * pow(rho0 * R * th0 / p_a, gamma);  // Eq. 3 at the background
+        ref3[t] = rho0;
+        ref3[FS + t] = th0;
+        ref3[2 * FS + t] = p_a * pow(rho0 * R * th0 / p_a, gamma);  // Eq. 3 at the background
     }
 }
 
@@ -275,7 +353,7 @@ __global__ void k_face_bc(const uint8_t *__restrict__ in, uint8_t *__restrict__ 
             snprintf(buf, sizeof buf, "%s:%d: %s: %s", __FILE__, __LINE__, #call,       \
                      cudaGetErrorString(e_));                                           \
             errstr = buf;                                                               \
-            goto cuda_fail;                                                             \
+            return false;                                                               \
         }                                                                               \
     } while (0)
 
@@ -285,6 +363,201 @@ static inline unsigned grid_for(int64_t n, int threads = 256, int64_t cap = 148 
     if (b > cap) b = cap;
     if (b < 1) b = 1;
     return (unsigned)b;
+}
+
+// Builds one DssLists set over `n_pos` positions.  scr/scr_end: device scratch (the not yet
+// written `met` region); small_tmp: fallback CUB temp storage of kSmallTmp bytes.
+// inv == nullptr: natural order (position = local node).
+static bool build_dss_lists(numa_ctx *c, DssLists &D, const int32_t *cg, int64_t n_pos,
+                            const int32_t *inv, char *scr, char *scr_end, char *small_tmp,
+                            cudaStream_t s, std::string &errstr)
+{
+    const int64_t NG = c->par.n_global;
+    {   // tiny meshes: the `met` region is smaller than the lists' scratch; use the fixed one
+        const size_t need_scr = 16 * (size_t)n_pos + 24 * (size_t)NG + 8 * 256;
+        if ((size_t)(scr_end - scr) < need_scr) {
+            if (need_scr > kSmallScr) { errstr = "internal: setup scratch does not fit"; return false; }
+            scr = small_tmp + kSmallTmp;
+            scr_end = scr + kSmallScr;
+        }
+    }
+    int32_t *keysA = (int32_t *)scr;
+    int32_t *keysB = keysA + n_pos;
+    int32_t *valsA = keysB + n_pos;
+    int32_t *valsB = valsA + n_pos;
+    char *after = (char *)align_up((size_t)(valsB + n_pos));
+    void *cub_tmp = (void *)after;
+    size_t cub_avail = after < scr_end ? (size_t)(scr_end - after) : 0;
+    if (cub_avail < kSmallTmp) { cub_tmp = small_tmp; cub_avail = kSmallTmp; }
+    if (after > scr_end) { errstr = "internal: setup scratch does not fit"; return false; }
+    k_sort_input<<<grid_for(n_pos), 256, 0, s>>>(valsA, keysA, cg, n_pos, NG, inv, c->shell.BS,
+                                                 c->shell.epb, c->Mn, c->par.n_elem);
+    CK(cudaGetLastError());
+    int end_bit = 1;
+    while (((int64_t)1 << end_bit) <= NG) ++end_bit;  // keys reach the sentinel NG
+    cub::DoubleBuffer<int32_t> dk(keysA, keysB), dv(valsA, valsB);
+    size_t need = 0;
+    CK(cub::DeviceRadixSort::SortPairs(nullptr, need, dk, dv, (int)n_pos, 0, end_bit, s));
+    if (need > cub_avail) { errstr = "internal: CUB scratch does not fit"; return false; }
+    CK(cub::DeviceRadixSort::SortPairs(cub_tmp, need, dk, dv, (int)n_pos, 0, end_bit, s));
+    k_find_starts<<<grid_for(n_pos), 256, 0, s>>>(dk.Current(), D.start, n_pos, NG);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(D.copies, dv.Current(), (size_t)n_pos * 4, cudaMemcpyDeviceToDevice, s));
+    c->launches += 4;
+    // --- SHARED global nodes (multiplicity >= 2), sorted by (chunk, multiplicity class, first
+    // copy), and the transposed per-class copy lists of the DSS kernel
+    SharedPred pred{D.start};
+    thrust::counting_iterator<int32_t> ids(0);
+    int32_t *d_num = c->d_flags + 8;
+    int32_t *nodesA = (int32_t *)after;                          // [NG]
+    int32_t *nodesB = nodesA + NG;                               // [NG]
+    uint64_t *kA = (uint64_t *)align_up((size_t)(nodesB + NG));  // [NG]
+    uint64_t *kB = kA + NG;
+    char *tmp2c = (char *)align_up((size_t)(kB + NG));
+    void *tmp2 = tmp2c;
+    if (tmp2c > scr_end) { errstr = "internal: setup scratch does not fit"; return false; }
+    size_t avail2 = (size_t)(scr_end - tmp2c), need2 = 0;
+    if (avail2 < kSmallTmp) { tmp2 = small_tmp; avail2 = kSmallTmp; }
+    CK(cub::DeviceSelect::If(nullptr, need2, ids, nodesA, d_num, (int)NG, pred, s));
+    if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; return false; }
+    CK(cub::DeviceSelect::If(tmp2, need2, ids, nodesA, d_num, (int)NG, pred, s));
+    int32_t h_num = 0;
+    CK(cudaMemcpyAsync(&h_num, d_num, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    D.n_shared = h_num;
+    D.n_seg = 0;
+    D.blocks = 0;
+    if (h_num == 0) return true;
+    k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, D.start, D.copies, kA, h_num);
+    CK(cudaGetLastError());
+    int end_bit2 = 35;
+    while (((int64_t)NUMA_DSS_CHUNK << (end_bit2 - 34)) < n_pos) ++end_bit2;
+    cub::DoubleBuffer<uint64_t> dk2(kA, kB);
+    cub::DoubleBuffer<int32_t> dv2(nodesA, nodesB);
+    CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, dk2, dv2, h_num, 0, end_bit2, s));
+    if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; return false; }
+    CK(cub::DeviceRadixSort::SortPairs(tmp2, need2, dk2, dv2, h_num, 0, end_bit2, s));
+    CK(cudaMemcpyAsync(D.sh_nodes, dv2.Current(), (size_t)h_num * 4, cudaMemcpyDeviceToDevice, s));
+    // segment heads (positions where (chunk, class) changes), ascending
+    const size_t max_seg = WsMaxSeg((size_t)n_pos);
+    int32_t *heads = dv2.Alternate();  // [<= h_num], free after the sort
+    int32_t *hi = (int32_t *)dk2.Alternate();  // [<= h_num] ints inside a free [NG] uint64 buffer
+    SegHeadPred hp{dk2.Current()};
+    CK(cub::DeviceSelect::If(nullptr, need2, ids, heads, d_num, h_num, hp, s));
+    if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; return false; }
+    CK(cub::DeviceSelect::If(tmp2, need2, ids, heads, d_num, h_num, hp, s));
+    int32_t n_seg = 0;
+    CK(cudaMemcpyAsync(&n_seg, d_num, 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if ((size_t)n_seg > max_seg) { errstr = "internal: DSS segment table does not fit"; return false; }
+    k_gather_hi<<<(n_seg + 255) / 256, 256, 0, s>>>(dk2.Current(), heads, hi, n_seg);
+    CK(cudaGetLastError());
+    std::vector<int32_t> h_heads(n_seg), h_hi(n_seg);
+    CK(cudaMemcpyAsync(h_heads.data(), heads, (size_t)n_seg * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(h_hi.data(), hi, (size_t)n_seg * 4, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    std::vector<DssSeg> h_seg(n_seg);
+    std::vector<int32_t> h_map;
+    int64_t idx_off = 0, blk = 0;
+    for (int k = 0; k < n_seg; ++k) {
+        DssSeg &sg = h_seg[k];
+        sg.node_off = h_heads[k];
+        sg.n = (k + 1 < n_seg ? h_heads[k + 1] : h_num) - h_heads[k];
+        sg.cls = h_hi[k] & 3;
+        sg.idx_base = idx_off;
+        sg.blk0 = (int32_t)blk;
+        sg.pad = 0;
+        if (sg.cls < 3) idx_off += (int64_t)sg.n * (2 << sg.cls);
+        const int nb = (sg.n + NUMA_DSS_THREADS - 1) / NUMA_DSS_THREADS;
+        h_map.insert(h_map.end(), nb, k);
+        blk += nb;
+    }
+    if ((size_t)blk > (size_t)NG / NUMA_DSS_THREADS + max_seg + 1 || idx_off > n_pos) {
+        errstr = "internal: DSS tables do not fit";
+        return false;
+    }
+    D.n_seg = n_seg;
+    D.blocks = blk;
+    CK(cudaMemcpyAsync(D.seg, h_seg.data(), (size_t)n_seg * sizeof(DssSeg), cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(D.blkmap, h_map.data(), (size_t)blk * 4, cudaMemcpyHostToDevice, s));
+    k_class_lists<<<(unsigned)blk, NUMA_DSS_THREADS, 0, s>>>(D.sh_nodes, D.start, D.copies, D.idx,
+                                                            D.seg, D.blkmap);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(s));  // h_seg / h_map are read by the copies above
+    c->launches += 6;
+    return true;
+}
+
+static void bind_lists(DssLists &D, char *ws, const DssOff &o)
+{
+    D.start = (int32_t *)(ws + o.start);
+    D.copies = (int32_t *)(ws + o.copies);
+    D.sh_nodes = (int32_t *)(ws + o.sh_nodes);
+    D.idx = (int32_t *)(ws + o.idx);
+    D.seg = (DssSeg *)(ws + o.seg);
+    D.blkmap = (int32_t *)(ws + o.blkmap);
+}
+
+static bool init_device_tables(numa_ctx *c, const WsLayout &L, char *ws, const double *xyz,
+                               const int32_t *intma_cg, const uint8_t *face_bc, const double *ref,
+                               const double *sponge, cudaStream_t s, numa_status &result,
+                               std::string &errstr)
+{
+    const numa_params *p = &c->par;
+    const int64_t NL = c->NL, NG = p->n_global;
+    int32_t h_flags[4] = {0, 0, 0, 0};
+    CK(cudaMemsetAsync(c->d_flags, 0, 256, s));
+    // ids are validated before any list is indexed with them
+    k_check_ids<<<grid_for(NL), 256, 0, s>>>(intma_cg, NL, NG, c->d_flags);
+    CK(cudaGetLastError());
+    c->launches++;
+    CK(cudaMemcpyAsync(h_flags, c->d_flags, 16, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    if (h_flags[1]) {
+        errstr = "numa_init_geometry: intma_cg entry outside [0, n_global)";
+        result = NUMA_ERR_ARG;
+        return false;
+    }
+    // block-shell tables (host-built once per (N, epb), tiny)
+    {
+        const ShellTables &T = shell_tables(p->N, c->shell.epb, c->shell.BS);
+        std::vector<int32_t> inv((size_t)c->shell.BS, -1);
+        for (size_t t = 0; t < T.pos.size(); ++t) inv[(size_t)T.pos[t]] = (int32_t)t;
+        for (int le = 0; le < c->shell.epb && le < 16; ++le) c->shell.first_pos[le] = T.pos[(size_t)le * c->Mn];
+        CK(cudaMemcpyAsync(c->shell.pos, T.pos.data(), T.pos.size() * 4, cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(c->shell.tab, T.tab.data(), T.tab.size() * 4, cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(ws + L.shell_inv, inv.data(), inv.size() * 4, cudaMemcpyHostToDevice, s));
+        CK(cudaStreamSynchronize(s));
+    }
+    // DSS lists of both index spaces; scratch = the `met` region (written afterwards)
+    char *scr = ws + L.met, *scr_end = ws + L.omega;
+    if (!build_dss_lists(c, c->dss_nat, intma_cg, NL, nullptr, scr, scr_end, ws + L.small_tmp, s, errstr))
+        return false;
+    if (!build_dss_lists(c, c->dss_int, intma_cg, c->shell.FS, (const int32_t *)(ws + L.shell_inv), scr,
+                         scr_end, ws + L.small_tmp, s, errstr))
+        return false;
+    // the holes of the block-shell tables (pad positions, elements past Ne) are never used, but
+    // keep them finite; then metrics and wJ (wJ parked in `omega`), omega = wJ / M via the lists
+    CK(cudaMemsetAsync(ws + L.met, 0, L.nat.start - L.met, s));
+    CK(launch_metrics(c, xyz, c->omega, s));
+    CK(launch_mass(c, s));
+    k_ref3<<<grid_for(NL), 256, 0, s>>>(ref, c->ref3, NL, p->p_a, p->R_gas, c->gamma, c->shell.pos,
+                                        c->shell.epb * (int)c->Mn, (int)c->shell.BS, c->shell.FS);
+    CK(cudaGetLastError());
+    if (sponge) CK(launch_to_shell(c, sponge, c->sponge, 1, s));
+    k_face_bc<<<(unsigned)((p->n_elem + 255) / 256), 256, 0, s>>>(face_bc, c->face_bc, p->n_elem,
+                                                                  c->d_flags);
+    CK(cudaGetLastError());
+    c->launches += 4;
+    CK(cudaMemcpyAsync(h_flags, c->d_flags, 16, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    c->has_walls = h_flags[2];
+    if (h_flags[0]) {
+        errstr = "numa_init_geometry: non-positive Jacobian determinant";
+        result = NUMA_ERR_NEG_JACOBIAN;
+        return false;
+    }
+    return true;
 }
 
 extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xyz,
@@ -320,10 +593,9 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
     numa_ctx *c = new (std::nothrow) numa_ctx();
     if (!c) { g_err = "out of host memory"; return NUMA_ERR_ARG; }
     cudaStream_t s = (cudaStream_t)stream;
-    std::string errstr;
-    numa_status result = NUMA_OK;
     char *ws = (char *)workspace;
     c->par = *p;
+    cudaGetDevice(&c->device);
     c->Nq = p->N + 1;
     c->Mn = (int64_t)c->Nq * c->Nq * c->Nq;
     c->NL = p->n_elem * c->Mn;
@@ -334,154 +606,23 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
     c->omega = (double *)(ws + L.omega);
     c->ref3 = (double *)(ws + L.ref3);
     c->sponge = sponge ? (double *)(ws + L.sponge) : nullptr;
-    c->dss_start = (int32_t *)(ws + L.start);
-    c->dss_copies = (int32_t *)(ws + L.copies);
-    c->sh_nodes = (int32_t *)(ws + L.sh_nodes);
-    c->dss_idx = (int32_t *)(ws + L.dss_idx);
-    c->dss_seg = (DssSeg *)(ws + L.dss_seg);
-    c->dss_blkmap = (int32_t *)(ws + L.dss_blkmap);
+    bind_lists(c->dss_nat, ws, L.nat);
+    bind_lists(c->dss_int, ws, L.shl);
+    c->shell = L.shell;
+    c->shell.pos = (int32_t *)(ws + L.shell_pos);
+    c->shell.tab = (uint32_t *)(ws + L.shell_tab);
     c->face_bc = (uint8_t *)(ws + L.face_bc);
     c->d_flags = (int32_t *)(ws + L.flags);
-    {
-        const int64_t NL = c->NL, NG = p->n_global;
-        int32_t h_flags[4] = {0, 0, 0, 0};
-        // --- DSS lists: stable radix sort of (global id, local index); scratch aliases `met`
-        char *scr = ws + L.met;
-        int32_t *keysA = (int32_t *)scr;
-        int32_t *keysB = keysA + NL;
-        int32_t *valsA = keysB + NL;
-        int32_t *valsB = valsA + NL;
-        void *cub_tmp = (void *)align_up((size_t)(valsB + NL));
-        size_t cub_avail = (char *)cub_tmp < ws + L.omega ? (size_t)((ws + L.omega) - (char *)cub_tmp) : 0;
-        if (cub_avail < kSmallTmp) { cub_tmp = ws + L.small_tmp; cub_avail = kSmallTmp; }
-        CK(cudaMemsetAsync(c->d_flags, 0, 256, s));
-        k_iota_check<<<grid_for(NL), 256, 0, s>>>(valsA, intma_cg, keysA, NL, NG, c->d_flags);
-        CK(cudaGetLastError());
-        c->launches++;
-        int end_bit = 1;
-        while (((int64_t)1 << end_bit) < NG) ++end_bit;
-        cub::DoubleBuffer<int32_t> dk(keysA, keysB), dv(valsA, valsB);
-        size_t need = 0;
-        CK(cub::DeviceRadixSort::SortPairs(nullptr, need, dk, dv, (int)NL, 0, end_bit, s));
-        if (need > cub_avail) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
-        CK(cub::DeviceRadixSort::SortPairs(cub_tmp, need, dk, dv, (int)NL, 0, end_bit, s));
-        k_find_starts<<<grid_for(NL), 256, 0, s>>>(dk.Current(), c->dss_start, NL, NG);
-        CK(cudaGetLastError());
-        CK(cudaMemcpyAsync(c->dss_copies, dv.Current(), NL * 4, cudaMemcpyDeviceToDevice, s));
-        // --- SHARED global nodes (multiplicity >= 2), sorted by (multiplicity class, first
-        // copy), and the transposed per-class copy lists of the DSS kernel.  Scratch: the part
-        // of the `met` region behind the first sort's buffers.
-        {
-            SharedPred pred{c->dss_start};
-            thrust::counting_iterator<int32_t> ids(0);
-            int32_t *d_num = c->d_flags + 8;
-            char *scr2 = (char *)align_up((size_t)(valsB + NL));
-            char *scr_end = ws + L.omega;
-            int32_t *nodesA = (int32_t *)scr2;                         // [NG]
-            int32_t *nodesB = nodesA + NG;                             // [NG]
-            uint64_t *kA = (uint64_t *)align_up((size_t)(nodesB + NG));  // [NG]
-            uint64_t *kB = kA + NG;
-            void *tmp2 = (void *)align_up((size_t)(kB + NG));
-            size_t avail2 = (char *)tmp2 < scr_end ? (size_t)(scr_end - (char *)tmp2) : 0, need2 = 0;
-            if ((char *)tmp2 > scr_end) { errstr = "internal: setup scratch does not fit"; goto cuda_fail; }
-            if (avail2 < kSmallTmp) { tmp2 = ws + L.small_tmp; avail2 = kSmallTmp; }
-            CK(cub::DeviceSelect::If(nullptr, need2, ids, nodesA, d_num, (int)NG, pred, s));
-            if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
-            CK(cub::DeviceSelect::If(tmp2, need2, ids, nodesA, d_num, (int)NG, pred, s));
-            int32_t h_num = 0;
-            CK(cudaMemcpyAsync(&h_num, d_num, 4, cudaMemcpyDeviceToHost, s));
-            CK(cudaStreamSynchronize(s));
-            c->n_shared = h_num;
-            c->n_seg = 0;
-            c->dss_blocks = 0;
-            if (h_num > 0) {
-                k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, c->dss_start, c->dss_copies, kA, h_num);
-                CK(cudaGetLastError());
-                int end_bit2 = 35;
-                while (((int64_t)NUMA_DSS_CHUNK << (end_bit2 - 34)) < NL) ++end_bit2;
-                cub::DoubleBuffer<uint64_t> dk2(kA, kB);
-                cub::DoubleBuffer<int32_t> dv2(nodesA, nodesB);
-                CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, dk2, dv2, h_num, 0, end_bit2, s));
-                if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
-                CK(cub::DeviceRadixSort::SortPairs(tmp2, need2, dk2, dv2, h_num, 0, end_bit2, s));
-                CK(cudaMemcpyAsync(c->sh_nodes, dv2.Current(), (size_t)h_num * 4, cudaMemcpyDeviceToDevice, s));
-                // segment heads (positions where (chunk, class) changes), ascending
-                int32_t *heads = dv2.Alternate();           // [<= h_num], free after the sort
-                int32_t *hi = heads + WsMaxSeg(NL);
-                SegHeadPred hp{dk2.Current()};
-                CK(cub::DeviceSelect::If(nullptr, need2, ids, heads, d_num, h_num, hp, s));
-                if (need2 > avail2) { errstr = "internal: CUB scratch does not fit"; goto cuda_fail; }
-                CK(cub::DeviceSelect::If(tmp2, need2, ids, heads, d_num, h_num, hp, s));
-                int32_t n_seg = 0;
-                CK(cudaMemcpyAsync(&n_seg, d_num, 4, cudaMemcpyDeviceToHost, s));
-                CK(cudaStreamSynchronize(s));
-                if ((size_t)n_seg > WsMaxSeg(NL)) { errstr = "internal: DSS segment table does not fit"; goto cuda_fail; }
-                k_gather_hi<<<(n_seg + 255) / 256, 256, 0, s>>>(dk2.Current(), heads, hi, n_seg);
-                CK(cudaGetLastError());
-                std::vector<int32_t> h_heads(n_seg), h_hi(n_seg);
-                CK(cudaMemcpyAsync(h_heads.data(), heads, (size_t)n_seg * 4, cudaMemcpyDeviceToHost, s));
-                CK(cudaMemcpyAsync(h_hi.data(), hi, (size_t)n_seg * 4, cudaMemcpyDeviceToHost, s));
-                CK(cudaStreamSynchronize(s));
-                std::vector<DssSeg> h_seg(n_seg);
-                std::vector<int32_t> h_map;
-                int64_t idx_off = 0, blk = 0;
-                for (int k = 0; k < n_seg; ++k) {
-                    DssSeg &sg = h_seg[k];
-                    sg.node_off = h_heads[k];
-                    sg.n = (k + 1 < n_seg ? h_heads[k + 1] : h_num) - h_heads[k];
-                    sg.cls = h_hi[k] & 3;
-                    sg.idx_base = idx_off;
-                    sg.blk0 = (int32_t)blk;
-                    sg.pad = 0;
-                    if (sg.cls < 3) idx_off += (int64_t)sg.n * (2 << sg.cls);
-                    const int nb = (sg.n + NUMA_DSS_THREADS - 1) / NUMA_DSS_THREADS;
-                    h_map.insert(h_map.end(), nb, k);
-                    blk += nb;
-                }
-                if ((size_t)blk > (size_t)NG / NUMA_DSS_THREADS + WsMaxSeg(NL) + 1 || idx_off > NL) {
-                    errstr = "internal: DSS tables do not fit"; goto cuda_fail;
-                }
-                c->n_seg = n_seg;
-                c->dss_blocks = blk;
-                CK(cudaMemcpyAsync(c->dss_seg, h_seg.data(), (size_t)n_seg * sizeof(DssSeg), cudaMemcpyHostToDevice, s));
-                CK(cudaMemcpyAsync(c->dss_blkmap, h_map.data(), (size_t)blk * 4, cudaMemcpyHostToDevice, s));
-                k_class_lists<<<(unsigned)blk, NUMA_DSS_THREADS, 0, s>>>(c->sh_nodes, c->dss_start, c->dss_copies,
-                                                                        c->dss_idx, c->dss_seg, c->dss_blkmap);
-                CK(cudaGetLastError());
-                CK(cudaStreamSynchronize(s));  // h_seg / h_map are read by the copies above
-                c->launches += 6;
-            }
-        }
-        // --- metrics and wJ (wJ parked in `omega`), then omega = wJ / M via the CSR lists.
-        // (the setup scratch aliased `met`; the stream order makes the reuse safe)
-        CK(launch_metrics(c, xyz, c->omega, s));
-        CK(launch_mass(c, s));
-        k_ref3<<<grid_for(NL), 256, 0, s>>>(ref, c->ref3, NL, p->p_a, p->R_gas, c->gamma);
-        CK(cudaGetLastError());
-        if (sponge) CK(cudaMemcpyAsync(c->sponge, sponge, NL * 8, cudaMemcpyDeviceToDevice, s));
-        k_face_bc<<<(unsigned)((p->n_elem + 255) / 256), 256, 0, s>>>(face_bc, c->face_bc, p->n_elem,
-                                                                      c->d_flags);
-        CK(cudaGetLastError());
-        c->launches += 6;
-        CK(cudaMemcpyAsync(h_flags, c->d_flags, 16, cudaMemcpyDeviceToHost, s));
-        CK(cudaStreamSynchronize(s));
-        c->has_walls = h_flags[2];
-        if (h_flags[1]) {
-            g_err = "numa_init_geometry: intma_cg entry outside [0, n_global)";
-            result = NUMA_ERR_ARG;
-        } else if (h_flags[0]) {
-            g_err = "numa_init_geometry: non-positive Jacobian determinant";
-            result = NUMA_ERR_NEG_JACOBIAN;
-        }
+    numa_status result = NUMA_ERR_CUDA;
+    std::string errstr;
+    if (!init_device_tables(c, L, ws, xyz, intma_cg, face_bc, ref, sponge, s, result, errstr)) {
+        g_err = errstr;
+        cudaGetLastError();
+        delete c;
+        return result;
     }
-    if (result != NUMA_OK) { delete c; return result; }
     *out = c;
     return NUMA_OK;
-cuda_fail:
-    g_err = errstr;
-    cudaGetLastError();
-    delete c;
-    return NUMA_ERR_CUDA;
 }
 
 #undef CK
@@ -503,10 +644,23 @@ static numa_status arg_fail(numa_ctx *ctx, const char *msg)
     return NUMA_ERR_ARG;
 }
 
+// a context is bound to the device that was current at numa_init_geometry
+static bool wrong_device(numa_ctx *ctx)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device) {
+        ctx->err = "the current CUDA device is not the one this context was created on";
+        cudaGetLastError();
+        return true;
+    }
+    return false;
+}
+
 extern "C" numa_status numa_rhs(numa_ctx *ctx, const double *q, double *rhs, void *stream)
 {
     if (!ctx || !q || !rhs) return arg_fail(ctx, "numa_rhs: NULL argument");
     if (q == rhs) return arg_fail(ctx, "numa_rhs: rhs must not alias q");
+    if (wrong_device(ctx)) return NUMA_ERR_ARG;
     CKC(launch_rhs(ctx, q, rhs, (cudaStream_t)stream));
     return NUMA_OK;
 }
@@ -515,7 +669,8 @@ extern "C" numa_status numa_dss_or_flux(numa_ctx *ctx, double *rhs, void *stream
 {
     if (!ctx || !rhs) return arg_fail(ctx, "numa_dss_or_flux: NULL argument");
     if (ctx->par.method != 0) { ctx->err = "DG face flux is not built"; return NUMA_ERR_UNSUPPORTED; }
-    CKC(launch_dss_classes(ctx, rhs, K_DSS, (cudaStream_t)stream));
+    if (wrong_device(ctx)) return NUMA_ERR_ARG;
+    CKC(launch_dss_classes(ctx, ctx->dss_nat, rhs, ctx->NL, K_DSS, (cudaStream_t)stream));
     return NUMA_OK;
 }
 
@@ -523,6 +678,7 @@ extern "C" numa_status numa_apply_sources(numa_ctx *ctx, const double *q, const 
                                           double *rhs, void *stream)
 {
     if (!ctx || !q || !rhs) return arg_fail(ctx, "numa_apply_sources: NULL argument");
+    if (wrong_device(ctx)) return NUMA_ERR_ARG;
     CKC(launch_sources(ctx, q, heating, rhs, (cudaStream_t)stream));
     return NUMA_OK;
 }
@@ -532,6 +688,7 @@ extern "C" numa_status numa_rk_stage(numa_ctx *ctx, double a0, double a1, double
                                      double *q_out, void *stream)
 {
     if (!ctx || !q0 || !qs || !rhs || !q_out) return arg_fail(ctx, "numa_rk_stage: NULL argument");
+    if (wrong_device(ctx)) return NUMA_ERR_ARG;
     CKC(launch_rk(ctx, a0, a1, b_dt, q0, qs, rhs, q_out, (cudaStream_t)stream));
     return NUMA_OK;
 }
@@ -539,26 +696,85 @@ extern "C" numa_status numa_rk_stage(numa_ctx *ctx, double a0, double a1, double
 // SSP-RK3 (Shu-Osher; Q11): (a0, a1, b)
 static const double kRK3[3][3] = {{1.0, 0.0, 1.0}, {0.75, 0.25, 0.25}, {1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0}};
 
-extern "C" numa_status numa_step_rk3(numa_ctx *ctx, double *q, void *scratch, const double *heating,
-                                     double dt, int32_t n_steps, void *stream)
+// One SSP-RK3 step on the block-shell buffers A (state of the step, in/out) and B (stage state):
+//   stage 1: B = A + dt L(A);  stage 2: B = 3/4 A + 1/4 B + 1/4 dt L(B);
+//   stage 3: A = 1/3 A + 2/3 B + 2/3 dt L(B).
+// Each stage: the volume kernel writes the update as DSS partial sums (a block reads its own
+// records before it writes them, so q_out may alias qs or q0), then the DSS completes the
+// shared nodes in place.
+static cudaError_t enqueue_step(numa_ctx *ctx, double *A, double *B, const double *heating, double dt,
+                                cudaStream_t s)
+{
+    for (int st = 0; st < 3; ++st) {
+        const double *qs = (st == 0) ? A : B;
+        double *qo = (st == 2) ? A : B;
+        cudaError_t e = launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, A, qs, heating, qo, s);
+        if (e != cudaSuccess) return e;
+        e = launch_dss_classes(ctx, ctx->dss_int, qo, ctx->shell.FS, K_FUSED_DSS, s);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const double *heating,
+                                 double dt, int32_t n_steps, void *stream, bool use_graph)
 {
     if (!ctx || !q || !scratch) return arg_fail(ctx, "numa_step_rk3: NULL argument");
     if (n_steps < 0 || ((uintptr_t)scratch & 255)) return arg_fail(ctx, "numa_step_rk3: bad n_steps or scratch alignment");
+    if (wrong_device(ctx)) return NUMA_ERR_ARG;
+    if (n_steps == 0) return NUMA_OK;
     cudaStream_t s = (cudaStream_t)stream;
-    double *q1 = (double *)scratch;
-    for (int step = 0; step < n_steps; ++step) {
-        // stage 1: q1 = q + dt L(q);  stage 2: q1 = 3/4 q + 1/4 q1 + 1/4 dt L(q1);
-        // stage 3: q  = 1/3 q + 2/3 q1 + 2/3 dt L(q1).  Each stage: the volume kernel writes the
-        // update as DSS partial sums (element-local, so q_out may alias qs or q0), then the DSS
-        // completes the shared nodes in place.
-        for (int st = 0; st < 3; ++st) {
-            const double *qs = (st == 0) ? q : q1;
-            double *qo = (st == 2) ? q : q1;
-            CKC(launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, q, qs, heating, qo, s));
-            CKC(launch_dss_classes(ctx, qo, K_FUSED_DSS, s));
-        }
+    double *A = (double *)scratch;
+    double *B = (double *)((char *)scratch + shell_state_bytes(ctx->shell));
+    double *H = nullptr;
+    CKC(launch_to_shell(ctx, q, A, 5, s));
+    if (heating) {
+        H = (double *)((char *)scratch + 2 * shell_state_bytes(ctx->shell));
+        CKC(launch_to_shell(ctx, heating, H, 1, s));
     }
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (use_graph) CKC(cudaStreamIsCapturing(s, &cap));
+    if (use_graph && !ctx->prof && cap == cudaStreamCaptureStatusNone) {
+        GraphKey &k = ctx->graph_key;
+        if (!ctx->graph || k.q != q || k.heat != heating || k.scratch != scratch || k.dt != dt || k.s != s) {
+            if (ctx->graph) { cudaGraphExecDestroy(ctx->graph); ctx->graph = nullptr; }
+            cudaGraph_t g = nullptr;
+            CKC(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+            const int64_t l0 = ctx->launches;
+            cudaError_t e = enqueue_step(ctx, A, B, H, dt, s);
+            ctx->launches = l0;  // capture enqueues nothing
+            cudaError_t e2 = cudaStreamEndCapture(s, &g);
+            if (e != cudaSuccess || e2 != cudaSuccess) {
+                if (g) cudaGraphDestroy(g);
+                CKC(e != cudaSuccess ? e : e2);
+            }
+            e = cudaGraphInstantiate(&ctx->graph, g, 0);
+            cudaGraphDestroy(g);
+            CKC(e);
+            k.q = q; k.heat = heating; k.scratch = scratch; k.dt = dt; k.s = s;
+        }
+        for (int step = 0; step < n_steps; ++step) {
+            CKC(cudaGraphLaunch(ctx->graph, s));
+            ctx->launches += 6;  // kernels replayed per step
+        }
+    } else {
+        for (int step = 0; step < n_steps; ++step) CKC(enqueue_step(ctx, A, B, H, dt, s));
+    }
+    CKC(launch_from_shell(ctx, A, q, 5, s));
     return NUMA_OK;
+}
+
+extern "C" numa_status numa_step_rk3(numa_ctx *ctx, double *q, void *scratch, const double *heating,
+                                     double dt, int32_t n_steps, void *stream)
+{
+    return step_rk3_impl(ctx, q, scratch, heating, dt, n_steps, stream, false);
+}
+
+extern "C" numa_status numa_step_rk3_graph(numa_ctx *ctx, double *q, void *scratch,
+                                           const double *heating, double dt, int32_t n_steps,
+                                           void *stream)
+{
+    return step_rk3_impl(ctx, q, scratch, heating, dt, n_steps, stream, true);
 }
 
 extern "C" numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heating_host,
@@ -568,6 +784,7 @@ extern "C" numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const d
     if (!ctx || !q_host || !d_q || !scratch) return arg_fail(ctx, "numa_step_rk3_host: NULL argument");
     if ((heating_host == nullptr) != (d_heating == nullptr))
         return arg_fail(ctx, "numa_step_rk3_host: heating_host and d_heating must both be given or both NULL");
+    if (wrong_device(ctx)) return NUMA_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     const size_t nb = (size_t)ctx->NL * 8;
     CKC(cudaMemcpyAsync(d_q, q_host, 5 * nb, cudaMemcpyHostToDevice, s));
@@ -583,12 +800,12 @@ extern "C" numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, doubl
 {
     if (!ctx || !out) return NUMA_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t NL = (size_t)ctx->NL;
     cudaError_t e;
-    switch (which) {
-        case 0: e = cudaMemcpyAsync(out, ctx->met, 9 * NL * 8, cudaMemcpyDeviceToDevice, s); break;
-        case 1: e = cudaMemcpyAsync(out, ctx->omega, NL * 8, cudaMemcpyDeviceToDevice, s); break;
-        case 2: e = cudaMemcpyAsync(out, ctx->ref3 + 2 * NL, NL * 8, cudaMemcpyDeviceToDevice, s); break;
+    numa_ctx *c = const_cast<numa_ctx *>(ctx);   // (launch counters only)
+    switch (which) {   // the tables are kept block-shell; handed out in natural order
+        case 0: e = launch_from_shell(c, ctx->met, out, 9, s); break;
+        case 1: e = launch_from_shell(c, ctx->omega, out, 1, s); break;
+        case 2: e = launch_from_shell(c, ctx->ref3 + 2 * ctx->shell.FS, out, 1, s); break;
         case 3: e = cudaMemcpyAsync(out, ctx->lgl.D, (size_t)ctx->Nq * ctx->Nq * 8, cudaMemcpyHostToDevice, s); break;
         case 4: e = cudaMemcpyAsync(out, ctx->lgl.w, (size_t)ctx->Nq * 8, cudaMemcpyHostToDevice, s); break;
         default: return NUMA_ERR_ARG;
@@ -632,15 +849,19 @@ extern "C" numa_status numa_profile_read(numa_ctx *ctx, int32_t kernel_id, doubl
 extern "C" const char *numa_kernel_name(int32_t kernel_id)
 {
     static const char *names[K_COUNT] = {"k_rhs (volume)", "k_dss", "k_sources", "k_rk",
-                                         "k_stage_volume (fused)", "k_stage_dss (fused)"};
+                                         "k_stage_volume (fused)", "k_stage_dss (fused)",
+                                         "k_shell_layout (natural <-> block-shell)"};
     return (kernel_id >= 0 && kernel_id < K_COUNT) ? names[kernel_id] : "";
 }
+
+extern "C" int32_t numa_kernel_count(void) { return K_COUNT; }
 
 extern "C" int64_t numa_launch_count(const numa_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 extern "C" numa_status numa_destroy(numa_ctx *ctx)
 {
     if (ctx) {
+        if (ctx->graph) cudaGraphExecDestroy(ctx->graph);
         for (auto &r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
         for (auto &e : ctx->pool) cudaEventDestroy(e);
     }

@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "../../include/numa_b200.h"
+#include "../../include/numa_b200_measure.h"
 
 #define NUMA_MAX_NQ 9
 
@@ -20,7 +21,7 @@ struct LglTables {
 };
 
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
-enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_COUNT = 6 };
+enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_COUNT = 7 };
 
 #ifndef NUMA_DSS_CHUNK
 #define NUMA_DSS_CHUNK 2048    // local nodes per DSS locality chunk (measured best of 256..2 M on cfg3)
@@ -40,35 +41,68 @@ struct DssSeg {
 
 struct ProfRec { int id; cudaEvent_t a, b; };
 
+// One set of deterministic-DSS lists over an index space of `n_pos` local positions (the
+// natural element-local order, or the block-shell order of the fused route).  CSR over global
+// nodes (copies ascending within a node) plus the form the DSS kernel reads: the SHARED nodes
+// (multiplicity >= 2) sorted by (chunk of NUMA_DSS_CHUNK positions holding their first copy,
+// multiplicity class, first copy); a SEGMENT is a run of equal (chunk, class).  Classes 0,1,2
+// = 2,4,8 copies keep their copy lists transposed in idx (copy a of node t of the segment at
+// idx_base + a*n + t); class 3 = any other multiplicity goes through the CSR lists.
+struct DssLists {
+    int32_t *start = nullptr;    // [NG+1]
+    int32_t *copies = nullptr;   // [NL]
+    int32_t *sh_nodes = nullptr; // [n_shared] global ids of the shared nodes, in kernel order
+    int32_t *idx = nullptr;      // [<= NL]
+    DssSeg *seg = nullptr;       // [n_seg]
+    int32_t *blkmap = nullptr;   // [blocks] segment of every thread block of the DSS kernel
+    int64_t n_shared = 0, n_seg = 0, blocks = 0;
+};
+
+// Block-shell layout of every per-node device array the library keeps or works on
+// internally (metric terms, omega, reference state, sponge; the state and heating of the fused
+// route): elements are taken in blocks of `epb` consecutive elements; a block record of BS
+// positions holds the block's nodes entity by entity (face interiors, edge interiors, corners
+// each as contiguous runs, element by element; interior nodes fill the gaps), so the copies of
+// shared nodes form long contiguous runs and the DSS touches whole 32-byte sectors.  The order
+// is chosen (numa_shell.cpp) so that the volume kernel's thread-per-position shared-memory
+// accesses are free of bank conflicts.
+struct ShellLayout {
+    int epb = 1;             // elements per block (= StageShape<N>::EPB)
+    int64_t BS = 0;          // positions per block record (EPB*Mn rounded up to whole warps)
+    int64_t n_blocks = 0;
+    int64_t FS = 0;          // field stride = n_blocks * BS
+    int32_t *pos = nullptr;  // device [epb*Mn]: (element of block, node) -> position
+    uint32_t *tab = nullptr; // device [BS]: thread slot -> packed (position lane, node) (numa_stage.cu)
+    int first_pos[16] = {0}; // position of node 0 of the le-th element of a block
+};
+
+struct GraphKey { const double *q = nullptr, *heat = nullptr; void *scratch = nullptr; double dt = 0.0; cudaStream_t s = nullptr; };
+
 struct numa_ctx {
     numa_params par;
+    int device = 0;
     int Nq;
     int64_t Mn, NL;
     double gamma;
     LglTables lgl;
     // device tables, all inside the caller's workspace
-    double *met;     // [9][NL]   d xi_a / d x_c
-    double *omega;   // [NL]      wJ / M
-    double *ref3;    // [3][NL]   rho0, theta0, p0
-    double *sponge;  // [NL] or nullptr
-    int32_t *dss_start;   // [NG+1]  CSR over global nodes
-    int32_t *dss_copies;  // [NL]    local indices, ascending within a node
-    int32_t *sh_nodes;    // [n_shared] global ids of SHARED nodes (multiplicity >= 2), ascending
-    int64_t n_shared;
-    // the same lists in the form the DSS kernel reads.  The shared nodes (sh_nodes) are sorted
-    // by (chunk of NUMA_DSS_CHUNK local nodes holding their first copy, multiplicity class,
-    // first copy); a SEGMENT is a run of equal (chunk, class).  Classes 0,1,2 = 2,4,8 copies
-    // keep their copy lists transposed in dss_idx (copy a of node t of the segment at
-    // idx_base + a*n + t); class 3 = any other multiplicity goes through the CSR lists.
-    int32_t *dss_idx;      // [<= NL]
-    DssSeg *dss_seg;       // [n_seg]
-    int32_t *dss_blkmap;   // [dss_blocks] segment of every thread block of the DSS kernel
-    int64_t n_seg, dss_blocks;
+    // (block-shell order, field stride shell.FS)
+    double *met;     // [9][FS]   d xi_a / d x_c
+    double *omega;   // [FS]      wJ / M
+    double *ref3;    // [3][FS]   rho0, theta0, p0
+    double *sponge;  // [FS] or nullptr
+    DssLists dss_nat;     // natural element-local order (numa_dss_or_flux, mass)
+    DssLists dss_int;     // block-shell order (fused stage)
+    ShellLayout shell;
     uint8_t *face_bc;     // [Ne][8] (padded to 8 bytes per element)
     int32_t *d_flags;     // [4] device error flags
     int has_walls;
+    bool attr_rhs = false, attr_stage = false;  // dynamic-shared-memory attribute set on this device
     int64_t launches;
     std::string err;
+    // CUDA graph of one SSP-RK3 step (numa_step_rk3_graph)
+    cudaGraphExec_t graph = nullptr;
+    GraphKey graph_key;
     // per-kernel event timing
     bool prof = false;
     std::vector<ProfRec> recs;
@@ -109,12 +143,24 @@ cudaError_t launch_sources(numa_ctx *c, const double *q, const double *heat, dou
                            cudaStream_t s);
 cudaError_t launch_rk(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
                       const double *qs, const double *rhs, double *qout, cudaStream_t s);
-// fused stage (numa_stage.cu): volume + sources + walls + RK written as DSS partial sums,
-// then the in-place DSS by multiplicity class (kernel_id = profiling slot)
+// fused stage (numa_stage.cu): volume + sources + walls + RK written as DSS partial sums into
+// the block-shell state, then the in-place DSS by multiplicity class.  q0, qs, qout are
+// block-shell arrays [5][shell.FS]; heat is block-shell [shell.FS] or nullptr.
 cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
                                 const double *qs, const double *heat, double *qout,
                                 cudaStream_t s);
-cudaError_t launch_dss_classes(numa_ctx *c, double *r, int kernel_id, cudaStream_t s);
+// in-place DSS of r[5][stride] over one list set (kernel_id = profiling slot)
+cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_t stride,
+                               int kernel_id, cudaStream_t s);
+// natural [nf][NL] <-> block-shell [nf][shell.FS]
+cudaError_t launch_to_shell(numa_ctx *c, const double *q_nat, double *q_int, int nf, cudaStream_t s);
+cudaError_t launch_from_shell(numa_ctx *c, const double *q_int, double *q_nat, int nf, cudaStream_t s);
+// elements per block of the fused volume kernel for order N (fixes the block-shell layout)
+int stage_epb(int N);
+// host (numa_shell.cpp): tables of the block-shell layout for (N, epb): pos[le*Mn + n] and the
+// packed thread-slot table tab[BS]
+void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
+                          std::vector<uint32_t> &tab);
 
 #ifdef __CUDACC__
 // No-flux wall projection at one node (A9): faces in order 0..5; n = -+ grad xi_a/|grad xi_a|.

@@ -2,10 +2,20 @@
 // Alg. 1-2), deterministic DSS (Alg. 3), pointwise sources + no-flux walls, RK stage update,
 // and the setup kernel for the metric terms.  FP64 everywhere.
 //
-// Layout: f[m][e][n], n = i + Nq*(j + Nq*k) (the paper's q_e(i,j,k,e,m), L205).
+// Layout of the API arrays: f[m][e][n], n = i + Nq*(j + Nq*k) (the paper's q_e(i,j,k,e,m), L205).
+// The library's own tables (met, omega, ref3, sponge) are kept in the block-shell order of the
+// fused route (ShellLayout); the kernels of this file reach them through shell_index().
 #include "numa_internal.cuh"
 
 namespace {
+
+// position of natural local node p in a block-shell array (ShellLayout, numa_internal.cuh)
+struct ShellMap { const int32_t *pos; int npb; int BS; int64_t FS; };
+__device__ __forceinline__ int64_t shell_index(const ShellMap &m, int64_t p)
+{
+    const int64_t b = p / m.npb;
+    return b * m.BS + __ldg(m.pos + (int)(p - b * m.npb));
+}
 
 template <int N>
 struct Shape {
@@ -153,7 +163,8 @@ template <int N>
 __global__ void __launch_bounds__(Shape<N>::THREADS)
 k_rhs(const double *__restrict__ q, const double *__restrict__ ref3,
       const double *__restrict__ met, const double *__restrict__ omega, double *__restrict__ rhs,
-      const __grid_constant__ LglTables tab, int64_t Ne, int64_t NL, double g, double gamma)
+      const __grid_constant__ LglTables tab, int64_t Ne, int64_t NL, double g, double gamma,
+      const ShellMap sm)
 {
     constexpr int Nq = Shape<N>::Nq, Mn = Shape<N>::Mn, EPB = Shape<N>::EPB;
     extern __shared__ double sh[];  // [EPB][9][Mn] + D[Nq*Nq]
@@ -166,27 +177,30 @@ k_rhs(const double *__restrict__ q, const double *__restrict__ ref3,
     double Di[Nq], Dj[Nq], Dk[Nq];
     load_D_rows<Nq>(tab, i, j, k, Di, Dj, Dk, sD);
     const int64_t p = e * Mn + n;
+    const int64_t t = valid ? shell_index(sm, p) : 0;   // the library's tables are block-shell
     double rhop = 0.0, rho0 = 1.0;
     double *she = sh + (le < EPB ? le : 0) * 9 * Mn;
     if (valid) {
         rhop = q[0 * NL + p];
-        rho0 = ref3[0 * NL + p];
+        rho0 = ref3[0 * sm.FS + t];
         node_prepass(rhop, q[1 * NL + p], q[2 * NL + p], q[3 * NL + p], q[4 * NL + p], rho0,
-                     ref3[1 * NL + p], ref3[1 * NL + e * Mn], ref3[2 * NL + p], gamma, she, Mn, n);
+                     ref3[1 * sm.FS + t], ref3[1 * sm.FS + shell_index(sm, e * Mn)], ref3[2 * sm.FS + t],
+                     gamma, she, Mn, n);
     }
     __syncthreads();
     if (!valid) return;
     double m[9];
 #pragma unroll
-    for (int c = 0; c < 9; ++c) m[c] = met[c * NL + p];
+    for (int c = 0; c < 9; ++c) m[c] = met[c * sm.FS + t];
     double S[5];
     node_tendency<N>(she, i, j, k, Di, Dj, Dk, m, rhop, rho0, g, S);
-    const double om = omega[p];
+    const double om = omega[t];
 #pragma unroll
     for (int c = 0; c < 5; ++c) rhs[c * NL + p] = om * S[c];
 }
 
 // mass: M = sum over copies of wJ (all global nodes), omega = wJ / M, in place on `om`
+// (block-shell array; start/copies = the block-shell list set)
 __global__ void k_mass(double *__restrict__ om, const int32_t *__restrict__ start,
                        const int32_t *__restrict__ copies, int64_t NG)
 {
@@ -205,7 +219,7 @@ template <int N>
 __global__ void k_sources(const double *__restrict__ q, const double *__restrict__ heat,
                           const double *__restrict__ beta, const double *__restrict__ met,
                           const uint8_t *__restrict__ face_bc, double *__restrict__ r,
-                          int64_t NL, double f_cor)
+                          int64_t NL, double f_cor, const ShellMap sm)
 {
     constexpr int Nq = N + 1, Mn = Nq * Nq * Nq;
     const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -219,7 +233,7 @@ __global__ void k_sources(const double *__restrict__ q, const double *__restrict
     ru += f_cor * v;
     rv -= f_cor * u;
     if (beta) {
-        const double b = beta[p];
+        const double b = beta[shell_index(sm, p)];
         ru -= b * u; rv -= b * v; rw -= b * q[3 * NL + p]; rt -= b * q[4 * NL + p];
     }
     const uint2 bcw = *reinterpret_cast<const uint2 *>(face_bc + e * 8);
@@ -228,8 +242,9 @@ __global__ void k_sources(const double *__restrict__ q, const double *__restrict
         uint8_t bc[8];
         *reinterpret_cast<uint2 *>(bc) = bcw;
         double m[9];
+        const int64_t t = shell_index(sm, p);
 #pragma unroll
-        for (int c = 0; c < 9; ++c) m[c] = met[c * NL + p];
+        for (int c = 0; c < 9; ++c) m[c] = met[c * sm.FS + t];
         wall_project<Nq>(bc, i, j, k, m, ru, rv, rw);
     }
     r[1 * NL + p] = ru; r[2 * NL + p] = rv; r[3 * NL + p] = rw; r[4 * NL + p] = rt;
@@ -252,7 +267,8 @@ __global__ void k_rk(double a0, double a1, double b_dt, const double *q0, const 
 template <int N>
 __global__ void __launch_bounds__(Shape<N>::THREADS)
 k_metrics(const double *__restrict__ xyz, double *__restrict__ met, double *__restrict__ wJ,
-          const __grid_constant__ LglTables tab, int64_t Ne, int64_t NL, int32_t *flags)
+          const __grid_constant__ LglTables tab, int64_t Ne, int64_t NL, int32_t *flags,
+          const ShellMap sm)
 {
     constexpr int Nq = Shape<N>::Nq, Mn = Shape<N>::Mn, EPB = Shape<N>::EPB;
     __shared__ double sh[EPB * 3 * Mn];
@@ -280,16 +296,22 @@ k_metrics(const double *__restrict__ xyz, double *__restrict__ met, double *__re
     const double J = xx * c0 + yx * c1 + zx * c2;
     if (!(J > 0.0)) atomicOr(flags, 1);
     const double iJ = 1.0 / J;
-    met[0 * NL + p] = c0 * iJ;
-    met[1 * NL + p] = c1 * iJ;
-    met[2 * NL + p] = c2 * iJ;
-    met[3 * NL + p] = (yz * zx - yx * zz) * iJ;
-    met[4 * NL + p] = (xx * zz - xz * zx) * iJ;
-    met[5 * NL + p] = (xz * yx - xx * yz) * iJ;
-    met[6 * NL + p] = (yx * ze - ye * zx) * iJ;
-    met[7 * NL + p] = (xe * zx - xx * ze) * iJ;
-    met[8 * NL + p] = (xx * ye - xe * yx) * iJ;
-    wJ[p] = tab.w[i] * tab.w[j] * tab.w[k] * J;
+    const int64_t t = shell_index(sm, p), F = sm.FS;   // tables are written in block-shell order
+    met[0 * F + t] = c0 * iJ;
+    met[1 * F + t] = c1 * iJ;
+    met[2 * F + t] = c2 * iJ;
+    met[3 * F + t] = (yz * zx - yx * zz) * iJ;
+    met[4 * F + t] = (xx * zz - xz * zx) * iJ;
+    met[5 * F + t] = (xz * yx - xx * yz) * iJ;
+    met[6 * F + t] = (yx * ze - ye * zx) * iJ;
+    met[7 * F + t] = (xe * zx - xx * ze) * iJ;
+    met[8 * F + t] = (xx * ye - xe * yx) * iJ;
+    wJ[t] = tab.w[i] * tab.w[j] * tab.w[k] * J;
+}
+
+static ShellMap shell_map(const numa_ctx *c)
+{
+    return ShellMap{c->shell.pos, c->shell.epb * (int)c->Mn, (int)c->shell.BS, c->shell.FS};
 }
 
 template <int N>
@@ -297,15 +319,15 @@ cudaError_t rhs_N(numa_ctx *c, const double *q, double *rhs, cudaStream_t s)
 {
     const int64_t blocks = (c->par.n_elem + Shape<N>::EPB - 1) / Shape<N>::EPB;
     constexpr size_t smem = sizeof(double) * (Shape<N>::EPB * 9 * Shape<N>::Mn + Shape<N>::Nq * Shape<N>::Nq);
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the attribute is per device: set once per context (contexts are bound to one device)
+    if (!c->attr_rhs) {
         cudaError_t e = cudaFuncSetAttribute(k_rhs<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        c->attr_rhs = true;
     }
     k_rhs<N><<<(unsigned)blocks, Shape<N>::THREADS, smem, s>>>(q, c->ref3, c->met, c->omega, rhs,
                                                                c->lgl, c->par.n_elem, c->NL,
-                                                               c->par.g, c->gamma);
+                                                               c->par.g, c->gamma, shell_map(c));
     return cudaGetLastError();
 }
 
@@ -314,7 +336,7 @@ cudaError_t metrics_N(numa_ctx *c, const double *xyz, double *wJ, cudaStream_t s
 {
     const int64_t blocks = (c->par.n_elem + Shape<N>::EPB - 1) / Shape<N>::EPB;
     k_metrics<N><<<(unsigned)blocks, Shape<N>::THREADS, 0, s>>>(xyz, c->met, wJ, c->lgl,
-                                                                c->par.n_elem, c->NL, c->d_flags);
+                                                                c->par.n_elem, c->NL, c->d_flags, shell_map(c));
     return cudaGetLastError();
 }
 
@@ -324,7 +346,7 @@ cudaError_t sources_N(numa_ctx *c, const double *q, const double *heat, double *
 {
     const int64_t blocks = (c->NL + 255) / 256;
     k_sources<N><<<(unsigned)blocks, 256, 0, s>>>(q, heat, c->sponge, c->met, c->face_bc, rhs,
-                                                  c->NL, c->par.f_cor);
+                                                  c->NL, c->par.f_cor, shell_map(c));
     return cudaGetLastError();
 }
 
@@ -358,7 +380,7 @@ cudaError_t launch_mass(numa_ctx *c, cudaStream_t s)
 {
     c->launches++;
     const int64_t blocks = (c->par.n_global + 255) / 256;
-    k_mass<<<(unsigned)blocks, 256, 0, s>>>(c->omega, c->dss_start, c->dss_copies,
+    k_mass<<<(unsigned)blocks, 256, 0, s>>>(c->omega, c->dss_int.start, c->dss_int.copies,
                                             c->par.n_global);
     return cudaGetLastError();
 }

@@ -3,6 +3,12 @@
 // writes the stage update as DSS partial sums; a second kernel sums the partial sums of the
 // shared nodes in place (Alg. 3) in fixed order.  FP64 everywhere.
 //
+// Every per-node array of this route (state q0 / qs / q_out, metric terms, omega, reference
+// state, sponge, heating) is stored in the BLOCK-SHELL layout (ShellLayout, numa_internal.cuh;
+// DESIGN.md 6): the copies of shared nodes form long contiguous runs, so the DSS kernel touches
+// whole 32-byte sectors, and the volume kernel runs its pointwise phases one thread per
+// POSITION of a block record -- every global access is a coalesced, 256-byte-aligned stream.
+//
 // Why this is the same result: with omega = wJ/M and DSS the sum over
 // the copies of a global node,
 //     q_out = a0 q0 + a1 qs + b_dt P( DSS(omega S) + src )
@@ -49,11 +55,9 @@ struct StageShape {
     static constexpr int ME = SK * Nq;  // padded nodes per element and field
     static constexpr int NF = 8;        // p', u, v, w, theta, Fx, Fy, Fz
     static constexpr int NODES = EPB * Mn;
-    // Thread t of a block works on node  align_down(node0, 16) + t  (wrapping around inside the
-    // block's THREADS-node window), so that every warp-wide 8-byte global access starts on a
-    // 128-byte line: two L1 wavefronts instead of four to five when (N+1)^3 is not a multiple
-    // of 16.  WRAP = whether node0 can be misaligned at all.
-    static constexpr bool WRAP = (NODES % 16) != 0;
+    // positions per block record (ShellLayout::BS): whole warps, so that every block record of
+    // every field starts on a 256-byte line
+    static constexpr int BS = (NODES + 31) / 32 * 32;
     // NPT nodes per thread in the pointwise phases: at high N a block of Mn threads would be
     // alone on its SM (registers, shared memory); half as many threads let two blocks overlap
     // their memory and compute phases.
@@ -77,8 +81,8 @@ struct StageShape {
     static constexpr int THR_OVR = (N == 5) ? STAGE_THREADS5 : (N == 6) ? STAGE_THREADS6 : (N == 8) ? STAGE_THREADS8 : 0;
     static constexpr int NPT = THR_OVR ? (NODES + THR_OVR - 1) / THR_OVR
                                        : (N >= STAGE_NPT_MINN) ? STAGE_NPT_HI : 1;
-    static constexpr int THREADS = THR_OVR ? THR_OVR : ((NODES + NPT - 1) / NPT + 31) / 32 * 32;
-    static constexpr int SLOTS = THREADS * NPT;  // >= NODES
+    static constexpr int THREADS = THR_OVR ? THR_OVR : ((BS / 32 + NPT - 1) / NPT) * 32;
+    static constexpr int SLOTS = THREADS * NPT;  // >= BS
     static constexpr int LINES = EPB * N2;  // lines per field and direction
     // field stride in shared memory: = 2 (mod 4) doubles, so that with the FIELD-FASTEST task
     // enumeration (lane -> field = T mod 8, line = T / 8) the 16 lanes of a half-warp hit 16
@@ -130,11 +134,14 @@ struct StageShape {
 };
 
 struct StageArgs {
+    // all per-node arrays are block-shell: [fields][GFS], GFS = n_blocks * BS
     const double *qs, *q0;
     double *qout;
     const double *ref3, *met, *omega, *heat, *beta;
+    const uint32_t *tab;     // [BS] thread slot -> position and node (ShellLayout::tab)
     const uint8_t *face_bc;
-    int64_t Ne, NL;
+    int64_t Ne, GFS;
+    int first_pos[16];       // position of node 0 of the le-th element of a block (Q7)
     double g, gamma, f_cor, a0, a1, b_dt;
     double eos[14];  // binomial(gamma, n), n = 1..14: (1+x)^gamma - 1 = sum_n eos[n-1] x^n
     int has_walls;
@@ -247,25 +254,24 @@ __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
 }
 
-// Pointwise role of a thread: slot -> node.  The SLOTS slots of a block are laid over the
-// 16-node-aligned window that starts at or before node0; the slots in front of node0 take the
-// window's tail.
-struct NodeIx { bool has; int n, i, j, k, sp; int64_t p; };
+// Pointwise role of a thread: slot -> position of the block record -> node, from the table
+// (bits 0-9 shared-memory index sp, 10-13 i, 14-17 j, 18-21 k, 22-25 element of the block,
+// 26-30 lane of the position inside its warp's 32 positions; all ones = no node).
+struct NodeIx { bool has; int le, i, j, k, sp; int64_t p; };
 
 template <class SH>
-__device__ __forceinline__ NodeIx node_ix(int slot, int64_t node0, int n_nodes)
+__device__ __forceinline__ NodeIx node_ix(const uint32_t *__restrict__ tab, int slot, int64_t rec,
+                                          int n_elems)
 {
-    int bn = slot - (SH::WRAP ? (int)(node0 & 15) : 0);  // node within the block
-    if (SH::WRAP && bn < 0) bn += SH::SLOTS;
     NodeIx x;
-    x.has = bn < n_nodes;
-    const int le = x.has ? bn / SH::Mn : 0;
-    x.n = x.has ? bn - le * SH::Mn : 0;
-    x.k = x.n / SH::N2;
-    x.j = (x.n - x.k * SH::N2) / SH::Nq;
-    x.i = x.n - x.k * SH::N2 - x.j * SH::Nq;
-    x.sp = le * SH::ME + x.i + SH::SJ * x.j + SH::SK * x.k;
-    x.p = node0 + bn;
+    const uint32_t w = (slot < SH::BS) ? __ldg(tab + slot) : 0xFFFFFFFFu;
+    x.sp = (int)(w & 1023u);
+    x.i = (int)((w >> 10) & 15u);
+    x.j = (int)((w >> 14) & 15u);
+    x.k = (int)((w >> 18) & 15u);
+    x.le = (int)((w >> 22) & 15u);
+    x.has = (w != 0xFFFFFFFFu) && (x.le < n_elems);
+    x.p = rec + (slot & ~31) + (int)((w >> 26) & 31u);
     return x;
 }
 
@@ -283,11 +289,11 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     double *sPF = smem + SH::SMEM_WORK / sizeof(double);  // [NPF][SLOTS] cp.async prefetch (PFS)
 
     const int tid = threadIdx.x;
-    const int64_t NL = A.NL;
-    const int64_t node0 = (int64_t)blockIdx.x * SH::NODES;
-    const int64_t rem = NL - node0;
-    const int n_nodes = rem < SH::NODES ? (int)rem : SH::NODES;  // ragged last block
-    const int n_lines = n_nodes / Nq;                            // = elements * N2
+    const int64_t NL = A.GFS;                                  // field stride of every array
+    const int64_t rec = (int64_t)blockIdx.x * SH::BS;          // this block's record
+    const int64_t e0 = (int64_t)blockIdx.x * SH::EPB;
+    const int n_elems = (A.Ne - e0 < SH::EPB) ? (int)(A.Ne - e0) : SH::EPB;  // ragged last block
+    const int n_lines = n_elems * N2;
 
     constexpr int NPT = SH::NPT;
     static_assert(!SH::PREFETCH || NPT == 1, "register prefetch only with one node per thread");
@@ -299,7 +305,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     const bool same = (A.q0 == A.qs);
 #pragma unroll
     for (int rr = 0; rr < NPT; ++rr) {
-        const NodeIx x = node_ix<SH>(tid + rr * SH::THREADS, node0, n_nodes);
+        const NodeIx x = node_ix<SH>(A.tab, tid + rr * SH::THREADS, rec, n_elems);
         const int64_t p = x.p;
         const int sp = x.sp;
         rho0[rr] = 1.0;
@@ -337,7 +343,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
         }
         rho0[rr] = __ldg(A.ref3 + p);
         const double th0 = __ldg(A.ref3 + NL + p), p0 = __ldg(A.ref3 + 2 * NL + p);
-        const double th0e = __ldg(A.ref3 + NL + (p - x.n));  // theta0 at the element's first node (Q7)
+        const double th0e = __ldg(A.ref3 + NL + rec + A.first_pos[x.le]);  // theta0 at the element's first node (Q7)
         const double xx = (qv[rr][0] * th0 + qv[rr][4] * rho0[rr] + qv[rr][0] * qv[rr][4]) / (rho0[rr] * th0);
         const double rho = rho0[rr] + qv[rr][0];
         sW[0 * FS + sp] = p0 * eos_ratio(xx, A.gamma, A.eos);
@@ -404,10 +410,10 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     // ---- phase C: chain rule, Eq. 1 tendencies, sources, walls, stage update (A5-A10) -------
 #pragma unroll
     for (int rr = 0; rr < NPT; ++rr) {
-    const NodeIx x = node_ix<SH>(tid + rr * SH::THREADS, node0, n_nodes);
+    const NodeIx x = node_ix<SH>(A.tab, tid + rr * SH::THREADS, rec, n_elems);
     if (!x.has) continue;
     const int64_t p = x.p;
-    const int sp = x.sp, n = x.n, i = x.i, j = x.j, k = x.k;
+    const int sp = x.sp, i = x.i, j = x.j, k = x.k;
     if constexpr (SH::PFS) {
         if (rr == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
         const double *d = sPF + (tid + rr * SH::THREADS);
@@ -475,7 +481,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     if (A.has_walls) {
         const bool on_face = (i == 0) | (i == Nq - 1) | (j == 0) | (j == Nq - 1) | (k == 0) | (k == Nq - 1);
         if (on_face) {
-            const int64_t e = (p - n) / Mn;
+            const int64_t e = e0 + x.le;
             const uint2 bcw = *reinterpret_cast<const uint2 *>(A.face_bc + e * 8);
             if (bcw.x | bcw.y) {
                 // copies made only on this rare path: the out-of-line call needs its operands in
@@ -579,23 +585,59 @@ k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict
     }
 }
 
+// natural [nf][NL] <-> block-shell [nf][GFS]; one thread per natural node, so the natural side
+// is coalesced and the shell side is a gather / scatter inside the block's record (run once
+// per numa_step_rk3 call, not per stage)
+template <bool TO_SHELL>
+__global__ void k_shell_layout(const double *__restrict__ src, double *__restrict__ dst,
+                               const int32_t *__restrict__ pos, int64_t NL, int64_t GFS, int BS,
+                               int nodes_per_block, int nf)
+{
+    const int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= NL) return;
+    const int64_t b = p / nodes_per_block;
+    const int bn = (int)(p - b * nodes_per_block);
+    const int64_t t = b * BS + __ldg(pos + bn);
+    for (int c = 0; c < nf; ++c) {
+        if (TO_SHELL) dst[c * GFS + t] = src[c * NL + p];
+        else dst[c * NL + p] = src[c * GFS + t];
+    }
+}
+
 template <int N>
 cudaError_t stage_launch(numa_ctx *c, const StageArgs &a, cudaStream_t s)
 {
     using SH = StageShape<N>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    if (!c->attr_stage) {   // per device: a context is bound to one device
         cudaError_t e = cudaFuncSetAttribute(k_stage_volume<N>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SH::SMEM);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        c->attr_stage = true;
     }
     const int64_t blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
+    if (c->shell.BS != SH::BS || c->shell.epb != SH::EPB) return cudaErrorInvalidValue;  // layout of this context
     k_stage_volume<N><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a, c->lgl);
     return cudaGetLastError();
 }
 
+template <int N>
+int epb_of() { return StageShape<N>::EPB; }
+
 }  // namespace
+
+int stage_epb(int N)
+{
+    switch (N) {
+        case 2: return epb_of<2>();
+        case 3: return epb_of<3>();
+        case 4: return epb_of<4>();
+        case 5: return epb_of<5>();
+        case 6: return epb_of<6>();
+        case 7: return epb_of<7>();
+        case 8: return epb_of<8>();
+        default: return 1;
+    }
+}
 
 cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
                                 const double *qs, const double *heat, double *qout, cudaStream_t s)
@@ -604,8 +646,10 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
     StageArgs a;
     a.qs = qs; a.q0 = q0; a.qout = qout;
     a.ref3 = c->ref3; a.met = c->met; a.omega = c->omega; a.heat = heat; a.beta = c->sponge;
+    a.tab = c->shell.tab;
+    for (int le = 0; le < 16; ++le) a.first_pos[le] = le < c->shell.epb ? c->shell.first_pos[le] : 0;
     a.face_bc = c->face_bc;
-    a.Ne = c->par.n_elem; a.NL = c->NL;
+    a.Ne = c->par.n_elem; a.GFS = c->shell.FS;
     a.g = c->par.g; a.gamma = c->gamma; a.f_cor = c->par.f_cor;
     a.a0 = a0; a.a1 = a1; a.b_dt = b_dt;
     a.has_walls = c->has_walls;
@@ -629,11 +673,30 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
     }
 }
 
-cudaError_t launch_dss_classes(numa_ctx *c, double *r, int kernel_id, cudaStream_t s)
+cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_t stride,
+                               int kernel_id, cudaStream_t s)
 {
-    if (c->dss_blocks == 0) return cudaSuccess;
+    if (L.blocks == 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
-    k_stage_dss<<<(unsigned)c->dss_blocks, dim3(NUMA_DSS_THREADS, 5 / NUMA_DSS_FPT), 0, s>>>(
-        r, c->dss_idx, c->dss_seg, c->dss_blkmap, c->sh_nodes, c->dss_start, c->dss_copies, c->NL);
+    k_stage_dss<<<(unsigned)L.blocks, dim3(NUMA_DSS_THREADS, 5 / NUMA_DSS_FPT), 0, s>>>(
+        r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start, L.copies, stride);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_to_shell(numa_ctx *c, const double *q_nat, double *q_int, int nf, cudaStream_t s)
+{
+    LaunchScope ls(c, K_LAYOUT, s);
+    const int npb = c->shell.epb * (int)c->Mn;
+    k_shell_layout<true><<<(unsigned)((c->NL + 255) / 256), 256, 0, s>>>(q_nat, q_int, c->shell.pos, c->NL,
+                                                                         c->shell.FS, (int)c->shell.BS, npb, nf);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_from_shell(numa_ctx *c, const double *q_int, double *q_nat, int nf, cudaStream_t s)
+{
+    LaunchScope ls(c, K_LAYOUT, s);
+    const int npb = c->shell.epb * (int)c->Mn;
+    k_shell_layout<false><<<(unsigned)((c->NL + 255) / 256), 256, 0, s>>>(q_int, q_nat, c->shell.pos, c->NL,
+                                                                          c->shell.FS, (int)c->shell.BS, npb, nf);
     return cudaGetLastError();
 }
