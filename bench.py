@@ -42,11 +42,32 @@ def parse_workload(name):
     raise SystemExit("unknown workload %r" % name)
 
 
+def f_face(N):
+    """Share of an element's nodes that lie on its faces."""
+    return 1.0 - ((N - 1.0) / (N + 1.0)) ** 3
+
+
 def b_alg_bytes(N, has_src):
-    """Algorithmic bytes per local node per RK stage."""
-    f_face = 1.0 - ((N - 1.0) / (N + 1.0)) ** 3
+    """Algorithmic bytes per local node per RK stage (fixed there):
+    8 [5 qs + 5*2/3 q0 + 9 grad xi + 1 omega + 2 (rho0, theta0) + n_src + 5 q_out] + 2*8*5*f_face."""
+    return volume_alg_bytes(N, has_src) + dss_alg_bytes(N)
+
+
+def volume_alg_bytes(N, has_src):
+    """The volume kernel's share of B_alg: everything except the DSS round trip."""
     n_src = 2 if has_src else 0
-    return 8.0 * (5 + 5 * (2.0 / 3.0) + 9 + 1 + 2 + n_src + 5) + 2 * 8 * 5 * f_face
+    return 8.0 * (5 + 5 * (2.0 / 3.0) + 9 + 1 + 2 + n_src + 5)
+
+
+def dss_alg_bytes(N):
+    """The DSS kernel's share of B_alg: face nodes of 5 fields read and written once."""
+    return 2 * 8 * 5 * f_face(N)
+
+
+def f_alg_flops(N):
+    """Algorithmic FP64 flop per local node per RK stage: 48 (N+1) for the 24
+    contractions + 207 for chain rule, tendencies, DSS, sources and the stage update."""
+    return 48.0 * (N + 1) + 207.0
 
 
 def measured_peaks():
@@ -56,6 +77,30 @@ def measured_peaks():
             d = json.load(f)
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def captured_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the
+    tracked ncu --set full summary profiles/traffic_r2.json (written from the capture named
+    there); None when no capture of this workload / kernel is tracked."""
+    path = os.path.join(ROOT, "profiles", "traffic_r2.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        e = d["workloads"][workload][kernel.split(" ")[0]]
+        return float(e["dram_bytes_per_launch"]), "profiles/traffic_r2.json (%s)" % e["capture"]
+    except Exception:
+        return None, None
+
+
+def set_omp_threads(n):
+    """Thread count of the oracle's OpenMP runtime (libgomp, already loaded by the oracle)."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
 
 
 class ClockSampler:
@@ -133,9 +178,15 @@ def cpu_sample_workload(config, N):
         wl.name, wl.mesh.nx, wl.mesh.ny, wl.mesh.nz, wl.mesh.n_local)
 
 
-def time_oracle(wl, steps, warmup):
+def time_oracle(wl, steps, warmup, threads=None):
+    """Seconds for `steps` SSP-RK3 steps of the oracle (as it stands) and the threads it used."""
     from oracle import oracle as orc
     o = orc.Oracle.from_workload(wl)
+    ncpu = os.cpu_count() or 1
+    want = threads or int(os.environ.get("OMP_NUM_THREADS", ncpu))
+    want = max(1, min(want, ncpu))
+    if not set_omp_threads(want):
+        want = int(os.environ.get("OMP_NUM_THREADS", ncpu))
     q = wl.q
     for _ in range(warmup):
         q = o.step_rk3(q, wl.dt, wl.heating)
@@ -143,9 +194,7 @@ def time_oracle(wl, steps, warmup):
     for _ in range(steps):
         q = o.step_rk3(q, wl.dt, wl.heating)
     t = time.perf_counter() - t0
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    cores = min(cores, os.cpu_count() or cores)
-    return t, cores
+    return t, want
 
 
 def max_over_ranks(x, device, world):
@@ -174,8 +223,10 @@ def run_reference(args):
     steps = max(1, min(args.steps, 5))
     warm = max(0, min(args.warmup, 1))
     t, cores = time_oracle(wl, steps, warm)
+    t1, _ = time_oracle(wl, max(1, min(steps, 2)), 0, threads=1)
     NL = wl.mesh.n_local
     value = 5.0 * NL * 3 * steps / t / 1e9
+    value_1 = 5.0 * NL * 3 * max(1, min(steps, 2)) / t1 / 1e9
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": 1e3 * t / steps, "higher_is_better": True,
@@ -183,7 +234,7 @@ def run_reference(args):
         "config": {"workload": wl.name, "sample_of": args.workload, "N": wl.mesh.N,
                    "local_nodes": NL, "integrator": "SSP-RK3", "dt": wl.dt},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": sample},
+                         "sample": sample, "single_thread": {"value": value_1, "cores": 1}},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -206,8 +257,8 @@ def run_gpu(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    config, N = parse_workload(args.workload)
-    wl = inputs.make_workload(config, N=N)
+    config, N_arg = parse_workload(args.workload)
+    wl = inputs.make_workload(config, N=N_arg)
     mesh = wl.mesh
     NL = mesh.n_local
     g = binding.Numa.from_workload(wl, device=str(dev))
@@ -222,27 +273,24 @@ def run_gpu(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    # ---- device-resident timing -------------------------------------------------------
+    # ---- device-resident timing (per-kernel event timing OFF) --------------------------------
     g.step_rk3(q, wl.dt, heat, args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)   # nvidia-smi needs a moment before its first sample; untimed
-    g.profile(True)
     l0 = g.launch_count
     ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
     barrier()
     wall0 = time.time()
     ev0.record(stream)
-    g.step_rk3(q, wl.dt, heat, args.steps)
+    g.step_rk3(q, wl.dt, heat, args.steps, graph=args.graph)
     ev1.record(stream)
     barrier()
     wall1 = time.time()
     ms = ev0.elapsed_time(ev1)
     launches = g.launch_count - l0
-    prof = g.profile_read()
-    g.profile(False)
     if rank == 0 and not any(wall0 <= t <= wall1 + 0.03 for (t, _) in sampler.rows):
         # very short timed region: keep the same load running until a sample has been taken
         n0 = len(sampler.rows)
@@ -253,6 +301,16 @@ def run_gpu(args):
     clocks = sampler.stop(wall0, wall1) if rank == 0 else None
     finite = bool(torch.isfinite(q).all().item())
     ms = max_over_ranks(ms, dev, world)
+
+    # ---- second pass: the per-kernel split (CUDA events around every launch) ----------------
+    g.profile(True)
+    g.step_rk3(q, wl.dt, heat, min(args.steps, 10))
+    prof = g.profile_read()
+    g.profile(False)
+    prof_steps = min(args.steps, 10)
+
+    # ---- FP64 ceiling of this device (DFMA micro-benchmark, numa_b200_measure.h) -------------
+    fp64_peak = g.fp64_peak_tflops(5) if rank == 0 else None
 
     # ---- end to end through the C ABI with host buffers ---------------------------------
     qh = torch.from_numpy(wl.q.copy()).pin_memory()
@@ -279,52 +337,69 @@ def run_gpu(args):
     value = whole_job_gdof_per_s(NL, args.steps, world, ms * 1e-3)
     e2e_value = whole_job_gdof_per_s(NL, e2e_steps, world, t_e2e)
 
-    # ---- roofline of the dominant kernel -------------------------------------------------
+    # ---- roofline: the STAGE against max(t_HBM, t_FP64) ------------------------
     peak, peak_src = measured_peaks()
     has_src = wl.heating is not None
-    balg = b_alg_bytes(mesh.N, has_src)
-    roofline = None
-    if prof:
-        dom = max(prof.items(), key=lambda kv: kv[1][0])
-        dom_ms, dom_n = dom[1]
-        # B_alg covers one whole stage (all kernels of a stage); the dominant kernel's own
-        # algorithmic share is reported as `kernel_bytes_per_node`.
-        kb = kernel_alg_bytes(dom[0], mesh.N, has_src)
-        achieved = kb * NL / (dom_ms / dom_n * 1e-3) / 1e9
-        stage_ms = ms / (3 * args.steps)
-        # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-        # (profiles/r1e_final_cfg3.md: dram__bytes_read.sum + dram__bytes_write.sum of a stage-1
-        # launch of k_stage_volume<4> on cfg3); other workloads have no capture -> null
-        traffic = 5.25e9 if (wl.name == "cfg3_tc_100x100x20_N4" and dom[0].startswith("k_stage_volume")) else None
-        roofline = {
-            "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": traffic,
-            "traffic_source": "profiles/r1e_final_cfg3.md (stage-1 launch: 200 algorithmic B/node = 5.00e9 B)" if traffic else None,
-            "kernel": dom[0],
-            "kernel_ms": dom_ms / dom_n, "kernel_share_of_step": dom_ms / ms,
-            "kernel_bytes_per_node": kb, "peak_source": peak_src,
-            "stage": {"b_alg_bytes_per_node": balg, "ms": stage_ms,
-                      "achieved": balg * NL / (stage_ms * 1e-3) / 1e9,
-                      "frac": balg * NL / (stage_ms * 1e-3) / 1e9 / peak},
-            "kernels": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
-                            "share_of_step": v[0] / ms} for k, v in prof.items()},
-        }
+    N = mesh.N
+    balg, falg = b_alg_bytes(N, has_src), f_alg_flops(N)
+    stage_ms = ms / (3 * args.steps)
+    hbm_achieved = balg * NL / (stage_ms * 1e-3) / 1e9             # GB/s, algorithmic
+    fp64_achieved = falg * NL / (stage_ms * 1e-3) / 1e12           # TFLOP/s, algorithmic
+    t_hbm = balg * NL / (peak * 1e9)
+    t_fp64 = falg * NL / (fp64_peak * 1e12) if fp64_peak else 0.0
+    bound = "hbm" if t_hbm >= t_fp64 else "fp64"
+    kernels = {}
+    for name, (kms, kn) in prof.items():
+        kb = kernel_alg_bytes(name, N, has_src)
+        per = kms / kn
+        traffic, tsrc = captured_traffic(wl.name, name)
+        kernels[name] = {"ms_per_launch": per, "launches_per_step": kn / prof_steps,
+                         "share_of_step": kms / prof_steps / (ms / args.steps),
+                         "alg_bytes_per_node": kb,
+                         "achieved": kb * NL / (per * 1e-3) / 1e9 if kb else None,
+                         "frac": kb * NL / (per * 1e-3) / 1e9 / peak if kb else None,
+                         "traffic": traffic, "traffic_source": tsrc}
+    stage_kernels = {k: v for k, v in kernels.items() if k.startswith("k_stage")}
+    dom = max(stage_kernels.items(), key=lambda kv: kv[1]["share_of_step"])[0] if stage_kernels else None
+    roofline = {
+        "bound": bound,
+        "achieved": hbm_achieved if bound == "hbm" else fp64_achieved * 1e3,
+        "peak": peak if bound == "hbm" else fp64_peak * 1e3,
+        "unit": "GB/s" if bound == "hbm" else "GFLOP/s",
+        "frac": max(t_hbm, t_fp64) / (stage_ms * 1e-3),
+        "traffic": kernels[dom]["traffic"] if dom else None,
+        "traffic_source": kernels[dom]["traffic_source"] if dom else None,
+        "what": "one RK stage = volume kernel + DSS kernel; frac = max(t_HBM, t_FP64) / t_stage with "
+                "B_alg, F_alg of SURVEY.md 8(d) and the measured peaks",
+        "stage_ms": stage_ms, "b_alg_bytes_per_node": balg, "f_alg_flops_per_node": falg,
+        "peak_source": peak_src,
+        "hbm": {"achieved_gbs": hbm_achieved, "peak_gbs": peak, "frac": hbm_achieved / peak},
+        "fp64": {"achieved_tflops": fp64_achieved, "peak_tflops": fp64_peak,
+                 "frac": fp64_achieved / fp64_peak if fp64_peak else None,
+                 "peak_source": "DFMA micro-benchmark of this run (numa_measure_fp64_peak)"},
+        "dominant_kernel": dom,
+        "kernels": kernels,
+    }
 
-    # ---- CPU baseline: the oracle on a bounded sample ------------------------------------
+    # ---- CPU baseline: the oracle on a bounded sample, all cores and one core ------------------
     cpu = None
     if not args.no_cpu_baseline:
-        swl, sample = cpu_sample_workload(config, N)
-        t_cpu, cores = time_oracle(swl, 2, 1)
-        cpu = {"value": 5.0 * swl.mesh.n_local * 3 * 2 / t_cpu / 1e9, "unit": UNIT, "cores": cores,
-               "kind": "oracle", "sample": sample + ", 2 RK3 steps after 1 warm-up"}
+        swl, sample = cpu_sample_workload(config, N_arg)
+        t_cpu, cores = time_oracle(swl, 5, 1)
+        t_cpu1, _ = time_oracle(swl, 2, 0, threads=1)
+        cpu = {"value": 5.0 * swl.mesh.n_local * 3 * 5 / t_cpu / 1e9, "unit": UNIT, "cores": cores,
+               "kind": "oracle", "sample": sample + ", 5 RK3 steps after 1 warm-up",
+               "single_thread": {"value": 5.0 * swl.mesh.n_local * 3 * 2 / t_cpu1 / 1e9, "cores": 1,
+                                 "sample": "same sample, 2 RK3 steps"}}
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRIC, "value": value if finite else None, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl.name, "N": mesh.N, "elements": [mesh.nx, mesh.ny, mesh.nz],
                    "local_nodes": NL, "integrator": "SSP-RK3 (3 RHS + 3 stage updates per step)",
                    "dt": wl.dt, "multi_gpu": "replicas only" if world > 1 else "single",
+                   "launch": "CUDA graph per step" if args.graph else "plain launches",
                    "l2": "inputs larger than L2" if 22 * NL * 8 > 4 * 126e6 else
                          "working set may be L2-resident (reported, not a roofline case)",
                    "finite": finite},
@@ -340,24 +415,24 @@ def run_gpu(args):
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    if not finite:
+        raise SystemExit("bench.py: the state is not finite after the timed steps; no value reported")
 
 
 def kernel_alg_bytes(name, N, has_src):
-    """Algorithmic bytes per local node per launch of one kernel."""
-    f_face = 1.0 - ((N - 1.0) / (N + 1.0)) ** 3
+    """Algorithmic bytes per local node per launch of one kernel, on SURVEY.md 8(d)'s terms (the
+    stage kernels split B_alg between them; the four-call kernels count their own arrays)."""
     n_src = 2 if has_src else 0
     if name.startswith("k_rhs"):
-        return 8.0 * (5 + 9 + 1 + 3 + 5)              # q, met, omega, ref3 in; rhs out
-    if name.startswith("k_dss"):
-        return 2 * 8.0 * 5 * f_face                   # face nodes read + written
+        return 8.0 * (5 + 9 + 1 + 2 + 5)              # q, grad xi, omega, rho0/theta0 in; rhs out
+    if name.startswith("k_dss") or name.startswith("k_stage_dss"):
+        return dss_alg_bytes(N)                       # face nodes read + written
     if name.startswith("k_sources"):
         return 8.0 * (4 + n_src + 4 + 4)              # u,v,w,theta', heat, beta, rhs in/out (4 fields)
     if name.startswith("k_rk"):
         return 8.0 * (5 + 5 * (2.0 / 3.0) + 5 + 5)    # q0 (2/3 of stages), qs, rhs in; q out
     if name.startswith("k_stage_volume"):
-        return 8.0 * (5 + 5 * (2.0 / 3.0) + 9 + 1 + 3 + n_src + 5)
-    if name.startswith("k_stage_dss"):
-        return 2 * 8.0 * 5 * f_face
+        return volume_alg_bytes(N, has_src)
     return 0.0
 
 
@@ -369,6 +444,8 @@ def main():
     ap.add_argument("--impl", default="numa_b200", choices=["numa_b200", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--graph", action="store_true",
+                    help="launch every step as one CUDA graph (numa_step_rk3_graph; configs 1-2)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl != "reference":
         args.warmup = 3

@@ -735,15 +735,28 @@ static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const 
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (use_graph) CKC(cudaStreamIsCapturing(s, &cap));
     if (use_graph && !ctx->prof && cap == cudaStreamCaptureStatusNone) {
+        // the legacy default stream cannot be captured: the graph then runs on a stream of the
+        // context, ordered after / before the caller's stream with events
+        cudaStream_t cs = s;
+        if (s == nullptr || s == cudaStreamLegacy) {
+            if (!ctx->gstream) {
+                CKC(cudaStreamCreateWithFlags(&ctx->gstream, cudaStreamNonBlocking));
+                CKC(cudaEventCreateWithFlags(&ctx->gev0, cudaEventDisableTiming));
+                CKC(cudaEventCreateWithFlags(&ctx->gev1, cudaEventDisableTiming));
+            }
+            cs = ctx->gstream;
+            CKC(cudaEventRecord(ctx->gev0, s));
+            CKC(cudaStreamWaitEvent(cs, ctx->gev0, 0));
+        }
         GraphKey &k = ctx->graph_key;
-        if (!ctx->graph || k.q != q || k.heat != heating || k.scratch != scratch || k.dt != dt || k.s != s) {
+        if (!ctx->graph || k.q != q || k.heat != heating || k.scratch != scratch || k.dt != dt || k.s != cs) {
             if (ctx->graph) { cudaGraphExecDestroy(ctx->graph); ctx->graph = nullptr; }
             cudaGraph_t g = nullptr;
-            CKC(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+            CKC(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
             const int64_t l0 = ctx->launches;
-            cudaError_t e = enqueue_step(ctx, A, B, H, dt, s);
+            cudaError_t e = enqueue_step(ctx, A, B, H, dt, cs);
             ctx->launches = l0;  // capture enqueues nothing
-            cudaError_t e2 = cudaStreamEndCapture(s, &g);
+            cudaError_t e2 = cudaStreamEndCapture(cs, &g);
             if (e != cudaSuccess || e2 != cudaSuccess) {
                 if (g) cudaGraphDestroy(g);
                 CKC(e != cudaSuccess ? e : e2);
@@ -751,11 +764,15 @@ static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const 
             e = cudaGraphInstantiate(&ctx->graph, g, 0);
             cudaGraphDestroy(g);
             CKC(e);
-            k.q = q; k.heat = heating; k.scratch = scratch; k.dt = dt; k.s = s;
+            k.q = q; k.heat = heating; k.scratch = scratch; k.dt = dt; k.s = cs;
         }
         for (int step = 0; step < n_steps; ++step) {
-            CKC(cudaGraphLaunch(ctx->graph, s));
+            CKC(cudaGraphLaunch(ctx->graph, cs));
             ctx->launches += 6;  // kernels replayed per step
+        }
+        if (cs != s) {
+            CKC(cudaEventRecord(ctx->gev1, cs));
+            CKC(cudaStreamWaitEvent(s, ctx->gev1, 0));
         }
     } else {
         for (int step = 0; step < n_steps; ++step) CKC(enqueue_step(ctx, A, B, H, dt, s));
@@ -862,6 +879,7 @@ extern "C" numa_status numa_destroy(numa_ctx *ctx)
 {
     if (ctx) {
         if (ctx->graph) cudaGraphExecDestroy(ctx->graph);
+        if (ctx->gstream) { cudaStreamDestroy(ctx->gstream); cudaEventDestroy(ctx->gev0); cudaEventDestroy(ctx->gev1); }
         for (auto &r : ctx->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
         for (auto &e : ctx->pool) cudaEventDestroy(e);
     }

@@ -103,6 +103,8 @@ struct numa_ctx {
     // CUDA graph of one SSP-RK3 step (numa_step_rk3_graph)
     cudaGraphExec_t graph = nullptr;
     GraphKey graph_key;
+    cudaStream_t gstream = nullptr;   // used when the caller's stream is the legacy default stream
+    cudaEvent_t gev0 = nullptr, gev1 = nullptr;
     // per-kernel event timing
     bool prof = false;
     std::vector<ProfRec> recs;
