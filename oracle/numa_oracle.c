@@ -469,3 +469,108 @@ void orc_rk_stage(long n, double a0, double a1, double b_dt, const double *q0, c
 #pragma omp parallel for schedule(static)
     for (long p = 0; p < n; ++p) q_out[p] = a0 * q0[p] + a1 * qs[p] + b_dt * r[p];
 }
+
+/* ------------------------------------------------------------------------------------
+ * NEXT-4  RI-velocity diagnostic (Eq. 18-22; readings Q25-Q29 of
+ * DESIGN.md).  Pins: tests/test_oracle_ri.py.
+ *
+ * orc_ri_area: horizontal quadrature weight of every local node,
+ *     a = w_i w_j |x_xi y_eta - x_eta y_xi|,
+ * the LGL quadrature (Eq. 8) of the level surface zeta = const of a
+ * column-preserving mesh (L162-L168); the integrals "int_x int_y ... dx dy" of Eq. 22 at
+ * a height z are sums over the local nodes of that level with this weight (Q26).
+ * ---------------------------------------------------------------------------------- */
+void orc_ri_area(int N, long Ne, const double *xyz, double *a)
+{
+    int Nq = N + 1;
+    long Mn = (long)Nq * Nq * Nq, NL = Ne * Mn;
+    double xi[64], w[64], D[64 * 64];
+    orc_lgl(N, xi, w);
+    orc_dmat(N, xi, D);
+    for (long e = 0; e < Ne; ++e) {
+        const double *x = xyz + 0 * NL + e * Mn, *y = xyz + 1 * NL + e * Mn;
+        for (int k = 0; k < Nq; ++k)
+            for (int j = 0; j < Nq; ++j)
+                for (int i = 0; i < Nq; ++i) {
+                    double xx, xe, xz, yx, ye, yz;
+                    ref_derivs_diff(Nq, D, x, i, j, k, &xx, &xe, &xz);
+                    ref_derivs_diff(Nq, D, y, i, j, k, &yx, &ye, &yz);
+                    a[e * Mn + NODE(i, j, k)] = w[i] * w[j] * fabs(xx * ye - xe * yx);
+                }
+    }
+}
+
+/* orc_ri_velocity, in the paper's order:
+ *  Eq. 22 (L352): per level l, x_c = sum a |u| x / sum a |u|, |u| = (u^2+v^2+w^2)^(1/2)
+ *      ("weighted center of the velocity magnitude field", vertically varying); a level
+ *      whose denominator is 0 has no centroid and takes no part (valid[l] = 0).
+ *  Eq. 21 (L346): u_theta = (I - e_r x e_r - e_z x e_z) u,  e_r = r/|r|,
+ *      r = (x - x_c, y - y_c, 0), e_z = (0,0,1);   Eq. 20: u_theta = |u_theta| (a norm).
+ *  Strip mean (L360-L364): arithmetic mean of u_theta over the POINTS of the strip
+ *      s eps <= r < (s+1) eps, eps = r_max / n_strip, at each level (50 equi-width strips,
+ *      L366).  A point = a unique global node (its first local copy, Q28); a point with
+ *      r = 0 has no e_r and is left out; points with r >= r_max are left out (Q29).
+ *  Eq. 18 (L338): u_RI = max over (strip, level) with at least one point.
+ *  scalars[0] = u_RI, scalars[1] = max over points of (u^2+v^2)^(1/2) ("maximum horizontal
+ *      velocity" of Fig. 9).
+ * ---------------------------------------------------------------------------------- */
+void orc_ri_velocity(long NL, long NG, const int32_t *intma_cg, const int32_t *level, int n_lev,
+                     int n_strip, double r_max, const double *xyz, const double *a,
+                     const double *q, double *centroid /* [n_lev][2] */, int32_t *valid /* [n_lev] */,
+                     double *ubar /* [n_lev][n_strip] */, int32_t *count /* [n_lev][n_strip] */,
+                     double *scalars /* [2] */)
+{
+    const double *x = xyz, *y = xyz + NL;
+    const double *u = q + 1 * NL, *v = q + 2 * NL, *w = q + 3 * NL;
+    double *num_x = (double *)calloc((size_t)n_lev, sizeof(double));
+    double *num_y = (double *)calloc((size_t)n_lev, sizeof(double));
+    double *den = (double *)calloc((size_t)n_lev, sizeof(double));
+    for (long p = 0; p < NL; ++p) {
+        int l = level[p];
+        double mag = sqrt(u[p] * u[p] + v[p] * v[p] + w[p] * w[p]);
+        num_x[l] += a[p] * mag * x[p];
+        num_y[l] += a[p] * mag * y[p];
+        den[l] += a[p] * mag;
+    }
+    for (int l = 0; l < n_lev; ++l) {
+        valid[l] = den[l] > 0.0;
+        centroid[2 * l + 0] = valid[l] ? num_x[l] / den[l] : 0.0;
+        centroid[2 * l + 1] = valid[l] ? num_y[l] / den[l] : 0.0;
+    }
+    for (long t = 0; t < (long)n_lev * n_strip; ++t) { ubar[t] = 0.0; count[t] = 0; }
+    char *seen = (char *)calloc((size_t)NG, 1);
+    double eps = r_max / n_strip, umax_h = 0.0;
+    for (long p = 0; p < NL; ++p) {
+        long I = intma_cg[p];
+        if (seen[I]) continue;   /* a point is a unique global node: its first local copy */
+        seen[I] = 1;
+        double uh = sqrt(u[p] * u[p] + v[p] * v[p]);
+        if (uh > umax_h) umax_h = uh;
+        int l = level[p];
+        if (!valid[l]) continue;
+        double rx = x[p] - centroid[2 * l + 0], ry = y[p] - centroid[2 * l + 1];
+        double r = sqrt(rx * rx + ry * ry);
+        if (!(r > 0.0) || !(r < r_max)) continue;
+        double er[3] = {rx / r, ry / r, 0.0}, ez[3] = {0.0, 0.0, 1.0};
+        double uu[3] = {u[p], v[p], w[p]};
+        double ur = uu[0] * er[0] + uu[1] * er[1] + uu[2] * er[2];
+        double uz = uu[0] * ez[0] + uu[1] * ez[1] + uu[2] * ez[2];
+        double t0 = uu[0] - ur * er[0] - uz * ez[0];
+        double t1 = uu[1] - ur * er[1] - uz * ez[1];
+        double t2 = uu[2] - ur * er[2] - uz * ez[2];
+        double ut = sqrt(t0 * t0 + t1 * t1 + t2 * t2);
+        int s = (int)floor(r / eps);
+        if (s >= n_strip) continue;
+        ubar[(long)l * n_strip + s] += ut;
+        count[(long)l * n_strip + s] += 1;
+    }
+    double uri = 0.0;
+    for (long t = 0; t < (long)n_lev * n_strip; ++t)
+        if (count[t] > 0) {
+            ubar[t] /= count[t];
+            if (ubar[t] > uri) uri = ubar[t];
+        }
+    scalars[0] = uri;
+    scalars[1] = umax_h;
+    free(seen); free(num_x); free(num_y); free(den);
+}

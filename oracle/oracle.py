@@ -61,6 +61,10 @@ def lib():
         L.orc_sources.argtypes = [C.c_long, _dp, _dp, _dp, C.c_double, _dp]
         L.orc_walls.argtypes = [C.c_long, C.c_long, C.POINTER(C.c_int64), _dp, _dp]
         L.orc_rk_stage.argtypes = [C.c_long, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
+        _ip = C.POINTER(C.c_int32)
+        L.orc_ri_area.argtypes = [C.c_int, C.c_long, _dp, _dp]
+        L.orc_ri_velocity.argtypes = [C.c_long, C.c_long, _ip, _ip, C.c_int, C.c_int, C.c_double,
+                                      _dp, _dp, _dp, _dp, _ip, _dp, _ip, _dp]
         _lib = L
     return _lib
 
@@ -153,6 +157,31 @@ def rk_stage(a0, a1, b_dt, q0, qs, r, out=None):
         out = np.empty_like(q0)
     lib().orc_rk_stage(q0.size, a0, a1, b_dt, _p(q0), _p(qs), _p(r), _p(out))
     return out
+
+
+def ri_area(N, xyz):
+    """Horizontal quadrature weight a[Ne][Mn] of the RI diagnostic (Q26)."""
+    xyz = _f64(xyz)
+    a = np.empty(xyz.shape[1:])
+    lib().orc_ri_area(N, xyz.shape[1], _p(xyz), _p(a))
+    return a
+
+
+def ri_velocity(N, xyz, intma_cg, n_global, level, n_lev, q, r_max, n_strip=50, area=None):
+    """RI-velocity diagnostic (Eq. 18-22): dict with u_ri, umax_h, centroid[n_lev][2],
+    valid[n_lev], ubar[n_lev][n_strip], count[n_lev][n_strip]."""
+    xyz = _f64(xyz); q = _f64(q)
+    intma_cg = np.ascontiguousarray(intma_cg, dtype=np.int32)
+    level = np.ascontiguousarray(level, dtype=np.int32)
+    a = ri_area(N, xyz) if area is None else _f64(area)
+    cen = np.empty((n_lev, 2)); valid = np.empty(n_lev, dtype=np.int32)
+    ubar = np.empty((n_lev, n_strip)); cnt = np.empty((n_lev, n_strip), dtype=np.int32)
+    sc = np.empty(2)
+    lib().orc_ri_velocity(intma_cg.size, int(n_global), _p(intma_cg, C.c_int32), _p(level, C.c_int32),
+                          int(n_lev), int(n_strip), float(r_max), _p(xyz), _p(a), _p(q), _p(cen),
+                          _p(valid, C.c_int32), _p(ubar), _p(cnt, C.c_int32), _p(sc))
+    return dict(u_ri=float(sc[0]), umax_h=float(sc[1]), centroid=cen, valid=valid, ubar=ubar,
+                count=cnt, area=a)
 
 
 class Oracle:

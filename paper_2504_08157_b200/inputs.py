@@ -205,6 +205,18 @@ def box_mesh(N, nx, ny, nz, extent, origin=(0.0, 0.0, 0.0), z_ratio=1.0, perturb
                 periodic=tuple(periodic))
 
 
+def node_levels(mesh: Mesh):
+    """Horizontal level of every local node: level[e][n] = ez*N + k (int32) and the number of
+    levels.  Index data only (like intma_cg): the nodes "at a height z" over which the RI
+    diagnostic integrates and averages (Eq. 19, 22; reading Q25)."""
+    N, Nq = mesh.N, mesh.N + 1
+    ez = np.arange(mesh.n_elem) % mesh.nz                       # e = ez + nz*(ex + nx*ey)
+    k = np.arange(mesh.Mn) // (Nq * Nq)
+    n_lev = mesh.nz * N + (0 if mesh.periodic[2] else 1)
+    lev = (ez[:, None] * N + k[None, :]) % n_lev
+    return np.ascontiguousarray(lev, dtype=np.int32), int(n_lev)
+
+
 # --------------------------------------------------------------------------------------
 # reference (background) states: hydrostatic, functions of z only (PAPER.md:L66)
 # --------------------------------------------------------------------------------------
