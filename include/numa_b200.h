@@ -187,6 +187,42 @@ numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heat
  */
 numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, double *out, void *stream);
 
+/*
+ * RI-velocity diagnostic (Eq. 18-22) on the device;
+ * the paper computes it on the CPU after copying the state back (L172).  Readings Q25-Q29 of
+ * DESIGN.md:
+ *   - "height z" = a horizontal node level: level[e][n] in [0, n_levels) names the level of
+ *     every local node (index data, like intma_cg);
+ *   - Eq. 22: centroid of a level x_c = sum a |u| x / sum a |u| over the level's local nodes,
+ *     |u| = (u^2+v^2+w^2)^(1/2), a = w_i w_j |x_xi y_eta - x_eta y_xi| the horizontal LGL
+ *     quadrature weight (column-preserving meshes, L162-L168); a level at rest has no
+ *     centroid and takes no part;
+ *   - Eq. 20-21: u_theta = |(I - e_r e_r - e_z e_z) u|, e_r = r/|r|, r = (x-x_c, y-y_c, 0);
+ *   - L360-L366: arithmetic mean of u_theta over the POINTS (unique global nodes; the first
+ *     local copy) with s eps <= r < (s+1) eps, eps = r_max / n_strips (the paper: 50 strips),
+ *     r = 0 and r >= r_max left out;  Eq. 18: u_RI = max over (level, strip) holding a point.
+ * Results are bitwise reproducible run to run (fixed-order centroid sums; the strip sums are
+ * accumulated in 64-bit fixed point, exact to 2^-56 m/s per point).
+ *
+ * numa_ri_init (synchronises `stream`): builds, in ri_workspace, the area weights from
+ *   xyz [3][Ne][Mn] and the level-sorted node and point lists.  The context must outlive the
+ *   numa_ri.  NUMA_ERR_ARG if a level entry is outside [0, n_levels) or n_strips > 1024.
+ * numa_ri_velocity (enqueue only): q [5][Ne][Mn] ->
+ *   ubar     [n_levels][n_strips]  strip means (0 where count = 0)
+ *   count    [n_levels][n_strips]  points per strip (int32)
+ *   centroid [3][..]: n_levels pairs (x_c, y_c), then n_levels flags 1.0 / 0.0 (has a centroid)
+ *   scalars  [3]: u_RI, max over points of (u^2+v^2)^(1/2) (Fig. 9's "maximum horizontal
+ *            velocity"), and 1.0 if some u_theta was NaN or >= 4096 m/s (left out), else 0.0
+ */
+typedef struct numa_ri numa_ri;
+size_t numa_ri_workspace_bytes(const numa_params *p, int32_t n_levels, int32_t n_strips);
+numa_status numa_ri_init(numa_ctx *ctx, const double *xyz, const int32_t *level, int32_t n_levels,
+                         int32_t n_strips, double r_max, void *ri_workspace, size_t workspace_bytes,
+                         void *stream, numa_ri **out);
+numa_status numa_ri_velocity(numa_ri *ri, const double *q, double *ubar, int32_t *count,
+                             double *centroid, double *scalars, void *stream);
+numa_status numa_ri_destroy(numa_ri *ri);
+
 numa_status numa_destroy(numa_ctx *ctx);
 
 /* Text of the last error of this context ("" if none).  ctx may be NULL: returns the text

@@ -22,7 +22,8 @@ STATUS = {0: "NUMA_OK", 1: "NUMA_ERR_ARG", 2: "NUMA_ERR_UNSUPPORTED", 3: "NUMA_E
 EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometry", "numa_rhs",
            "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
            "numa_step_rk3_graph", "numa_step_rk3_host", "numa_copy_table", "numa_destroy",
-           "numa_last_error"]
+           "numa_last_error", "numa_ri_workspace_bytes", "numa_ri_init", "numa_ri_velocity",
+           "numa_ri_destroy"]
 MEASURE_EXPORTS = ["numa_profile_enable", "numa_profile_read", "numa_kernel_name",
                    "numa_kernel_count", "numa_launch_count", "numa_measure_fp64_peak"]
 
@@ -68,6 +69,12 @@ def load_library(path: str | None = None):
     L.numa_step_rk3_graph.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
     L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
+    L.numa_ri_workspace_bytes.argtypes = [C.POINTER(NumaParams), C.c_int32, C.c_int32]
+    L.numa_ri_workspace_bytes.restype = C.c_size_t
+    L.numa_ri_init.argtypes = [vp, dp, dp, C.c_int32, C.c_int32, C.c_double, vp, C.c_size_t, vp,
+                               C.POINTER(vp)]
+    L.numa_ri_velocity.argtypes = [vp, dp, dp, dp, dp, dp, vp]
+    L.numa_ri_destroy.argtypes = [vp]
     L.numa_profile_enable.argtypes = [vp, C.c_int32]
     L.numa_profile_enable.restype = C.c_int
     L.numa_profile_read.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -85,7 +92,7 @@ def load_library(path: str | None = None):
     L.numa_last_error.restype = C.c_char_p
     for f in ("numa_init_geometry", "numa_rhs", "numa_dss_or_flux", "numa_apply_sources",
               "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_graph", "numa_step_rk3_host",
-              "numa_copy_table",
+              "numa_copy_table", "numa_ri_init", "numa_ri_velocity", "numa_ri_destroy",
               "numa_destroy"):
         getattr(L, f).restype = C.c_int
     if path is None:
@@ -223,6 +230,32 @@ class Numa:
         self.apply_sources(q, heating, r)
         return r
 
+    # -- RI-velocity diagnostic (numa_ri_*) ---------------------------------------------------
+    def ri_init(self, xyz, level, n_levels, r_max, n_strips=50):
+        """numa_ri_init: area weights and level-sorted lists into a torch workspace."""
+        xyz_d = _dev(xyz, torch.float64, self.device)
+        lev_d = _dev(level, torch.int32, self.device)
+        n = self.lib.numa_ri_workspace_bytes(C.byref(self.params), n_levels, n_strips)
+        if n == 0:
+            raise NumaError(1, "numa_ri_workspace_bytes: parameters out of range")
+        self._ri_ws = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._ri = C.c_void_p()
+        self._ri_shape = (int(n_levels), int(n_strips))
+        self._check(self.lib.numa_ri_init(self.ctx, _ptr(xyz_d), _ptr(lev_d), n_levels, n_strips,
+                                          float(r_max), _ptr(self._ri_ws), n, _stream(),
+                                          C.byref(self._ri)))
+
+    def ri_velocity(self, q):
+        """numa_ri_velocity -> (ubar[n_lev][n_strip], count, centroid[3*n_lev], scalars[3]) on the device."""
+        nl, ns = self._ri_shape
+        ubar = torch.empty((nl, ns), dtype=torch.float64, device=self.device)
+        count = torch.empty((nl, ns), dtype=torch.int32, device=self.device)
+        cen = torch.empty(3 * nl, dtype=torch.float64, device=self.device)
+        sc = torch.empty(3, dtype=torch.float64, device=self.device)
+        self._check(self.lib.numa_ri_velocity(self._ri, _ptr(q), _ptr(ubar), _ptr(count), _ptr(cen),
+                                              _ptr(sc), _stream()))
+        return ubar, count, cen, sc
+
     def profile(self, enable=True):
         self._check(self.lib.numa_profile_enable(self.ctx, 1 if enable else 0))
 
@@ -249,6 +282,9 @@ class Numa:
         return int(self.lib.numa_launch_count(self.ctx))
 
     def close(self):
+        if getattr(self, "_ri", None) is not None and self._ri.value:
+            self.lib.numa_ri_destroy(self._ri)
+            self._ri = C.c_void_p()
         if getattr(self, "ctx", None) is not None and self.ctx.value:
             self.lib.numa_destroy(self.ctx)
             self.ctx = C.c_void_p()

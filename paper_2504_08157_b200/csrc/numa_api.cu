@@ -596,6 +596,7 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
     char *ws = (char *)workspace;
     c->par = *p;
     cudaGetDevice(&c->device);
+    if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->n_sm < 1) c->n_sm = 148;
     c->Nq = p->N + 1;
     c->Mn = (int64_t)c->Nq * c->Nq * c->Nq;
     c->NL = p->n_elem * c->Mn;

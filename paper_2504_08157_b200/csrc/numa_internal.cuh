@@ -81,6 +81,7 @@ struct GraphKey { const double *q = nullptr, *heat = nullptr; void *scratch = nu
 struct numa_ctx {
     numa_params par;
     int device = 0;
+    int n_sm = 148;   // multiprocessors of `device` (grid of the persistent kernels)
     int Nq;
     int64_t Mn, NL;
     double gamma;
