@@ -188,6 +188,33 @@ numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heat
 numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, double *out, void *stream);
 
 /*
+ * Tensor-based hyper-diffusion (Section 2.4, Eq. 14-16,
+ * L139-L154): H_q = (-1)^(alpha+1) (div tau grad)^alpha q with alpha = 2 on u, v, w, theta'
+ * (H_u, H_theta of Eq. 1b-1c; rho' has none).  Readings Q30-Q33 of DESIGN.md:
+ *   - L f = div(tau grad f) element-locally in the strong chain-rule form of the rest of the
+ *     path, assembled as every tendency: H = -DSS(omega L( DSS(omega L q) )), tau entering each
+ *     application (L145);
+ *   - Eq. 15-16 with the element size along the i-th principal axis dx_i = 2 lambda_i^(1/2):
+ *     tau = 4 dt_ref^(-1/2) J E diag(c_i^(1/2)) E^T J^T, E = eigenvectors of G = J^-1 J^-T by
+ *     ASCENDING eigenvalue (c_1 acts along the longest principal axis of the element, c_3 along
+ *     the shortest).  Where two eigenvalues coincide (e.g. hx = hy) the matching c_i must be
+ *     equal, otherwise tau depends on an arbitrary choice of eigenvectors;
+ *   - H is added to the assembled velocity / theta' tendency before the no-flux projection.
+ *
+ * numa_hd_init (enqueue only): builds tau[6] at every node from the stored metric terms into
+ *   hd_workspace (>= numa_hd_workspace_bytes, 256-byte aligned, caller-owned, must outlive its
+ *   use) and switches hyper-diffusion on for this context (all c_i = 0 switches it off):
+ *   numa_step_rk3 / _graph / _host then include H in every stage (three more launches and one
+ *   more 4-field DSS per stage).  c3 = (c_1, c_2, c_3) >= 0 dimensionless, dt_ref = the dt of Eq. 16.
+ * numa_hyperdiffusion (enqueue only): the four-call route's step, to be called between
+ *   numa_dss_or_flux and numa_apply_sources: rhs[1..4] += H(q), q and rhs [5][Ne][Mn].
+ */
+size_t numa_hd_workspace_bytes(const numa_params *p);
+numa_status numa_hd_init(numa_ctx *ctx, const double *c3, double dt_ref, void *hd_workspace,
+                         size_t workspace_bytes, void *stream);
+numa_status numa_hyperdiffusion(numa_ctx *ctx, const double *q, double *rhs, void *stream);
+
+/*
  * RI-velocity diagnostic (Eq. 18-22) on the device;
  * the paper computes it on the CPU after copying the state back (L172).  Readings Q25-Q29 of
  * DESIGN.md:
@@ -200,7 +227,7 @@ numa_status numa_copy_table(const numa_ctx *ctx, int32_t which, double *out, voi
  *   - Eq. 20-21: u_theta = |(I - e_r e_r - e_z e_z) u|, e_r = r/|r|, r = (x-x_c, y-y_c, 0);
  *   - L360-L366: arithmetic mean of u_theta over the POINTS (unique global nodes; the first
  *     local copy) with s eps <= r < (s+1) eps, eps = r_max / n_strips (the paper: 50 strips),
- *     r = 0 and r >= r_max left out;  Eq. 18: u_RI = max over (level, strip) holding a point.
+ *     r >= r_max left out, e_r := 0 at r = 0;  Eq. 18: u_RI = max over (level, strip) holding a point.
  * Results are bitwise reproducible run to run (fixed-order centroid sums; the strip sums are
  * accumulated in 64-bit fixed point, exact to 2^-56 m/s per point).
  *

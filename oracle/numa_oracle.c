@@ -509,7 +509,8 @@ void orc_ri_area(int N, long Ne, const double *xyz, double *a)
  *  Strip mean (L360-L364): arithmetic mean of u_theta over the POINTS of the strip
  *      s eps <= r < (s+1) eps, eps = r_max / n_strip, at each level (50 equi-width strips,
  *      L366).  A point = a unique global node (its first local copy, Q28); a point with
- *      r = 0 has no e_r and is left out; points with r >= r_max are left out (Q29).
+ *      r = 0 has no radial direction, nothing radial is removed there (e_r := 0) and it
+ *      belongs to strip 0; points with r >= r_max are left out (Q29).
  *  Eq. 18 (L338): u_RI = max over (strip, level) with at least one point.
  *  scalars[0] = u_RI, scalars[1] = max over points of (u^2+v^2)^(1/2) ("maximum horizontal
  *      velocity" of Fig. 9).
@@ -550,8 +551,9 @@ void orc_ri_velocity(long NL, long NG, const int32_t *intma_cg, const int32_t *l
         if (!valid[l]) continue;
         double rx = x[p] - centroid[2 * l + 0], ry = y[p] - centroid[2 * l + 1];
         double r = sqrt(rx * rx + ry * ry);
-        if (!(r > 0.0) || !(r < r_max)) continue;
-        double er[3] = {rx / r, ry / r, 0.0}, ez[3] = {0.0, 0.0, 1.0};
+        if (!(r < r_max)) continue;
+        double er[3] = {0.0, 0.0, 0.0}, ez[3] = {0.0, 0.0, 1.0};
+        if (r > 0.0) { er[0] = rx / r; er[1] = ry / r; }
         double uu[3] = {u[p], v[p], w[p]};
         double ur = uu[0] * er[0] + uu[1] * er[1] + uu[2] * er[2];
         double uz = uu[0] * ez[0] + uu[1] * ez[1] + uu[2] * ez[2];
@@ -573,4 +575,69 @@ void orc_ri_velocity(long NL, long NG, const int32_t *intma_cg, const int32_t *l
     scalars[0] = uri;
     scalars[1] = umax_h;
     free(seen); free(num_x); free(num_y); free(den);
+}
+
+/* ------------------------------------------------------------------------------------
+ * NEXT-1  Tensor-based hyper-diffusion (Section 2.4, Eq. 14-16;
+ * readings Q30-Q33 of DESIGN.md).  H_q = (-1)^(alpha+1) (div tau grad)^alpha q with
+ * alpha = 2 (L145): H_q = - L(L(q)),  L f = div( tau grad f ), tau applied in EACH
+ * application of the Laplacian (L145 "multiplying the viscosity tensor tau by each
+ * application of the Laplacian operator").  The viscosity tensor tau (Eq. 15-16) is built in
+ * oracle.py with LAPACK's symmetric eigensolver as the library step.
+ *
+ * orc_hd_laplacian: element-local strong form, in the same style as Alg. 1-2 (Q2, Q30):
+ *   g   = grad f           (Alg. 2 reference derivatives + chain rule with grad xi_a)
+ *   F   = tau g            (tau[6][NL] = xx, xy, xz, yy, yz, zz at every local node)
+ *   out = div F            (9 reference derivatives + chain rule), for nf fields.
+ * The assembly between and after the two applications (omega weight + DSS, Eq. 11-12) is
+ * done by the caller with orc_weight / orc_dss.  Pins: tests/test_oracle_hyperdiffusion.py.
+ * ---------------------------------------------------------------------------------- */
+void orc_hd_laplacian(int N, long Ne, int nf, const double *met, const double *tau, const double *f,
+                      double *out)
+{
+    int Nq = N + 1;
+    long Mn = (long)Nq * Nq * Nq, NL = Ne * Mn;
+    double xi[64], w[64], D[64 * 64];
+    orc_lgl(N, xi, w);
+    orc_dmat(N, xi, D);
+#pragma omp parallel
+    {
+        double *F = (double *)malloc(sizeof(double) * 3 * Mn);
+#pragma omp for schedule(static)
+        for (long e = 0; e < Ne; ++e) {
+            long b = e * Mn;
+            for (int m = 0; m < nf; ++m) {
+                const double *fe = f + (long)m * NL + b;
+                for (int k = 0; k < Nq; ++k)
+                    for (int j = 0; j < Nq; ++j)
+                        for (int i = 0; i < Nq; ++i) {
+                            long n = NODE(i, j, k), p = b + n;
+                            double fx, fy, fz, g[3];
+                            ref_derivs(Nq, D, fe, i, j, k, &fx, &fy, &fz);
+                            for (int c = 0; c < 3; ++c)
+                                g[c] = fx * met[(0 + c) * NL + p] + fy * met[(3 + c) * NL + p] +
+                                       fz * met[(6 + c) * NL + p];
+                            double txx = tau[0 * NL + p], txy = tau[1 * NL + p], txz = tau[2 * NL + p],
+                                   tyy = tau[3 * NL + p], tyz = tau[4 * NL + p], tzz = tau[5 * NL + p];
+                            F[0 * Mn + n] = txx * g[0] + txy * g[1] + txz * g[2];
+                            F[1 * Mn + n] = txy * g[0] + tyy * g[1] + tyz * g[2];
+                            F[2 * Mn + n] = txz * g[0] + tyz * g[1] + tzz * g[2];
+                        }
+                for (int k = 0; k < Nq; ++k)
+                    for (int j = 0; j < Nq; ++j)
+                        for (int i = 0; i < Nq; ++i) {
+                            long p = b + NODE(i, j, k);
+                            double div = 0.0;
+                            for (int c = 0; c < 3; ++c) {
+                                double fx, fy, fz;
+                                ref_derivs(Nq, D, F + c * Mn, i, j, k, &fx, &fy, &fz);
+                                div += fx * met[(0 + c) * NL + p] + fy * met[(3 + c) * NL + p] +
+                                       fz * met[(6 + c) * NL + p];
+                            }
+                            out[(long)m * NL + p] = div;
+                        }
+            }
+        }
+        free(F);
+    }
 }

@@ -61,6 +61,7 @@ def lib():
         L.orc_sources.argtypes = [C.c_long, _dp, _dp, _dp, C.c_double, _dp]
         L.orc_walls.argtypes = [C.c_long, C.c_long, C.POINTER(C.c_int64), _dp, _dp]
         L.orc_rk_stage.argtypes = [C.c_long, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
+        L.orc_hd_laplacian.argtypes = [C.c_int, C.c_long, C.c_int, _dp, _dp, _dp, _dp]
         _ip = C.POINTER(C.c_int32)
         L.orc_ri_area.argtypes = [C.c_int, C.c_long, _dp, _dp]
         L.orc_ri_velocity.argtypes = [C.c_long, C.c_long, _ip, _ip, C.c_int, C.c_int, C.c_double,
@@ -159,6 +160,40 @@ def rk_stage(a0, a1, b_dt, q0, qs, r, out=None):
     return out
 
 
+def hd_tau(met, c, dt):
+    """Viscosity tensor of the hyper-diffusion (Eq. 15-16) at every local
+    node, from the metric terms met[9][Ne][Mn] (row a = grad xi_a, i.e. the matrix J^-1):
+        G = J^-1 J^-T (L149);  eigenvalues of G ascending = (1/lambda_1, 1/lambda_2, 1/lambda_3),
+        E = eigenvectors in columns (LAPACK dsyevd through numpy.linalg.eigh: the library step);
+        nu_i = c_i^(1/alpha) dx_i^2 / dt^(1/alpha), alpha = 2 (Eq. 16), with the element size in
+        the i-th principal direction taken as dx_i = 2 lambda_i^(1/2) (reading Q31: the
+        reference element [-1,1] has length 2, so an axis-aligned brick gets dx_i = h_i);
+        tau = J E diag(nu_i / lambda_i) (J E)^T (Eq. 15).
+    Returns tau[6][Ne][Mn] = (xx, xy, xz, yy, yz, zz)."""
+    met = _f64(met)
+    shp = met.shape[1:]
+    Jinv = np.moveaxis(met.reshape(3, 3, -1), 2, 0)          # [node][a][c] = d xi_a / d x_c
+    J = np.linalg.inv(Jinv)                                   # d x_c / d xi_a  ([node][c][a])
+    G = Jinv @ np.swapaxes(Jinv, 1, 2)                        # J^-1 J^-T
+    ev, E = np.linalg.eigh(G)                                 # ascending eigenvalues 1/lambda_i
+    lam = 1.0 / ev
+    dx = 2.0 * np.sqrt(lam)
+    nu = np.sqrt(np.asarray(c, dtype=np.float64))[None, :] * dx ** 2 / np.sqrt(dt)
+    JE = J @ E
+    T = (JE * (nu / lam)[:, None, :]) @ np.swapaxes(JE, 1, 2)
+    T = 0.5 * (T + np.swapaxes(T, 1, 2))
+    out = np.stack([T[:, 0, 0], T[:, 0, 1], T[:, 0, 2], T[:, 1, 1], T[:, 1, 2], T[:, 2, 2]])
+    return np.ascontiguousarray(out.reshape((6,) + shp))
+
+
+def hd_laplacian(N, met, tau, f):
+    """Element-local L f = div(tau grad f) for f[nf][Ne][Mn] (strong form, Q30)."""
+    f = _f64(f)
+    out = np.empty_like(f)
+    lib().orc_hd_laplacian(N, f.shape[1], f.shape[0], _p(_f64(met)), _p(_f64(tau)), _p(f), _p(out))
+    return out
+
+
 def ri_area(N, xyz):
     """Horizontal quadrature weight a[Ne][Mn] of the RI diagnostic (Q26)."""
     xyz = _f64(xyz)
@@ -188,7 +223,7 @@ class Oracle:
     """A0 once, then rhs()/step_rk3() on element-local SoA arrays [m][Ne][Mn]."""
 
     def __init__(self, N, xyz, intma_cg, n_global, face_bc, ref, constants, f_cor=0.0,
-                 sponge=None):
+                 sponge=None, hd_c=None, hd_dt=1.0):
         self.N = N
         self.intma_cg = np.ascontiguousarray(intma_cg, dtype=np.int32)
         self.n_global = int(n_global)
@@ -202,12 +237,26 @@ class Oracle:
             raise ValueError("non-positive Jacobian at %d nodes" % bad)
         self.wJ, self.M, self.omega = mass(N, self.intma_cg, self.n_global, self.jac)
         self.wall_node, self.wall_normal = wall_list(N, face_bc, self.met)
+        # NEXT-1: tensor hyper-diffusion (Eq. 14-16), off unless coefficients are given
+        self.tau = None
+        if hd_c is not None and any(float(x) != 0.0 for x in hd_c):
+            self.tau = hd_tau(self.met, hd_c, hd_dt)
 
     @classmethod
-    def from_workload(cls, wl):
+    def from_workload(cls, wl, hd_c=None, hd_dt=1.0):
         m = wl.mesh
         return cls(m.N, m.xyz, m.intma_cg, m.n_global, m.face_bc, wl.ref, wl.constants,
-                   f_cor=wl.f_cor, sponge=wl.sponge)
+                   f_cor=wl.f_cor, sponge=wl.sponge, hd_c=hd_c, hd_dt=hd_dt)
+
+    def hyperdiffusion(self, q):
+        """H_q = -L(L(q)) on u, v, w, theta' (Eq. 14 with alpha = 2; Eq. 1b-1c), L = M^-1 DSS(wJ
+        div(tau grad .)) (Eq. 11-12): two applications with the assembly after each.  [4][Ne][Mn]."""
+        f = np.ascontiguousarray(_f64(q)[1:5])
+        l1 = weight(self.omega, hd_laplacian(self.N, self.met, self.tau, f))
+        dss(self.intma_cg, self.n_global, l1)
+        l2 = weight(self.omega, hd_laplacian(self.N, self.met, self.tau, l1))
+        dss(self.intma_cg, self.n_global, l2)
+        return -l2
 
     # --- the separate calls of the C-ABI boundary -------------------------------------
     def rhs_local(self, q, want_T=False):
@@ -223,8 +272,10 @@ class Oracle:
         return dss(self.intma_cg, self.n_global, r)
 
     def apply_sources(self, q, heat, r):
-        """numa_apply_sources: A8 then A9, in place."""
+        """numa_apply_sources: A8 (+ H_q of Eq. 1b-1c when enabled) then A9, in place."""
         sources(q, heat, self.sponge, self.f_cor, r)
+        if self.tau is not None:
+            r[1:5] += self.hyperdiffusion(q)
         walls(self.wall_node, self.wall_normal, r)
         return r
 

@@ -23,7 +23,7 @@ EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometr
            "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
            "numa_step_rk3_graph", "numa_step_rk3_host", "numa_copy_table", "numa_destroy",
            "numa_last_error", "numa_ri_workspace_bytes", "numa_ri_init", "numa_ri_velocity",
-           "numa_ri_destroy"]
+           "numa_ri_destroy", "numa_hd_workspace_bytes", "numa_hd_init", "numa_hyperdiffusion"]
 MEASURE_EXPORTS = ["numa_profile_enable", "numa_profile_read", "numa_kernel_name",
                    "numa_kernel_count", "numa_launch_count", "numa_measure_fp64_peak"]
 
@@ -69,6 +69,10 @@ def load_library(path: str | None = None):
     L.numa_step_rk3_graph.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
     L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
+    L.numa_hd_workspace_bytes.argtypes = [C.POINTER(NumaParams)]
+    L.numa_hd_workspace_bytes.restype = C.c_size_t
+    L.numa_hd_init.argtypes = [vp, C.POINTER(C.c_double), C.c_double, vp, C.c_size_t, vp]
+    L.numa_hyperdiffusion.argtypes = [vp, dp, dp, vp]
     L.numa_ri_workspace_bytes.argtypes = [C.POINTER(NumaParams), C.c_int32, C.c_int32]
     L.numa_ri_workspace_bytes.restype = C.c_size_t
     L.numa_ri_init.argtypes = [vp, dp, dp, C.c_int32, C.c_int32, C.c_double, vp, C.c_size_t, vp,
@@ -93,7 +97,7 @@ def load_library(path: str | None = None):
     for f in ("numa_init_geometry", "numa_rhs", "numa_dss_or_flux", "numa_apply_sources",
               "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_graph", "numa_step_rk3_host",
               "numa_copy_table", "numa_ri_init", "numa_ri_velocity", "numa_ri_destroy",
-              "numa_destroy"):
+              "numa_hd_init", "numa_hyperdiffusion", "numa_destroy"):
         getattr(L, f).restype = C.c_int
     if path is None:
         _LIB = L
@@ -223,10 +227,24 @@ class Numa:
                                                 dt, n_steps, _stream()))
         return q_host
 
+    def hd_init(self, c3, dt_ref):
+        """numa_hd_init: tensor hyper-diffusion (Eq. 14-16) on; c3 = (c_1, c_2, c_3)."""
+        n = self.lib.numa_hd_workspace_bytes(C.byref(self.params))
+        self._hd_ws = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._hd = True
+        c = (C.c_double * 3)(*[float(x) for x in c3])
+        self._check(self.lib.numa_hd_init(self.ctx, c, float(dt_ref), _ptr(self._hd_ws), n, _stream()))
+
+    def hyperdiffusion(self, q, r):
+        self._check(self.lib.numa_hyperdiffusion(self.ctx, _ptr(q), _ptr(r), _stream()))
+        return r
+
     def full_rhs(self, q, heating=None):
-        """Convenience: the four separate calls that form L(q)."""
+        """Convenience: the separate calls that form L(q) (with H_q when hd_init was called)."""
         r = self.rhs(q)
         self.dss_or_flux(r)
+        if getattr(self, "_hd", False):
+            self.hyperdiffusion(q, r)
         self.apply_sources(q, heating, r)
         return r
 

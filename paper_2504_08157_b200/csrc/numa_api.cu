@@ -125,7 +125,10 @@ struct WsLayout {
     ShellLayout shell;  // sizes only (pos = nullptr)
 };
 
-static inline size_t WsMaxSeg(size_t n_pos) { return 4 * (n_pos / NUMA_DSS_CHUNK + 2); }
+static inline size_t WsMaxSeg(size_t n_pos) { return 4 * (n_pos / NUMA_DSS_CHUNK + 2); }   // sized for the smaller chunk
+// positions per DSS locality chunk: measured on the block-shell layout (cfg3 / cfg4, ms per launch)
+//   N=4: 0.69 / 0.53 / 0.53 / 0.55 at 512 / 2048 / 8192 / 32768;  N=7: 0.70 / 0.55 / 0.50 / 0.48;  N=8: 0.67 / 0.54 / 0.49 / 0.46
+static inline int64_t dss_chunk(int N) { return N <= 4 ? NUMA_DSS_CHUNK : NUMA_DSS_CHUNK_HI; }
 
 static bool params_ok(const numa_params *p)
 {
@@ -276,7 +279,7 @@ struct SharedPred {
 // class 0,1,2 = 2,4,8 copies, 3 = anything else.
 __global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *__restrict__ start,
                              const int32_t *__restrict__ copies, uint64_t *__restrict__ keys,
-                             int64_t n)
+                             int64_t n, uint32_t chunk)
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
@@ -288,7 +291,7 @@ __global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *_
         const uint64_t cls = (c == 2) ? 0 : (c == 4) ? 1 : (c == 8) ? 2 : 3;
 #endif
         const uint32_t first = (uint32_t)copies[s];
-        keys[t] = ((uint64_t)(first / NUMA_DSS_CHUNK) << 34) | (cls << 32) | first;
+        keys[t] = ((uint64_t)(first / chunk) << 34) | (cls << 32) | first;
     }
 }
 
@@ -428,10 +431,11 @@ static bool build_dss_lists(numa_ctx *c, DssLists &D, const int32_t *cg, int64_t
     D.n_seg = 0;
     D.blocks = 0;
     if (h_num == 0) return true;
-    k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, D.start, D.copies, kA, h_num);
+    const uint32_t chunk = (uint32_t)dss_chunk(c->par.N);
+    k_class_keys<<<grid_for(h_num), 256, 0, s>>>(nodesA, D.start, D.copies, kA, h_num, chunk);
     CK(cudaGetLastError());
     int end_bit2 = 35;
-    while (((int64_t)NUMA_DSS_CHUNK << (end_bit2 - 34)) < n_pos) ++end_bit2;
+    while (((int64_t)chunk << (end_bit2 - 34)) < n_pos) ++end_bit2;
     cub::DoubleBuffer<uint64_t> dk2(kA, kB);
     cub::DoubleBuffer<int32_t> dv2(nodesA, nodesB);
     CK(cub::DeviceRadixSort::SortPairs(nullptr, need2, dk2, dv2, h_num, 0, end_bit2, s));
@@ -709,7 +713,14 @@ static cudaError_t enqueue_step(numa_ctx *ctx, double *A, double *B, const doubl
     for (int st = 0; st < 3; ++st) {
         const double *qs = (st == 0) ? A : B;
         double *qo = (st == 2) ? A : B;
-        cudaError_t e = launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, A, qs, heating, qo, s);
+        cudaError_t e = cudaSuccess;
+        // hyper-diffusion (Eq. 14, alpha = 2): first application from qs before qo (which may alias
+        // qs) is written; second application added to the partial sums before the stage's DSS
+        if (ctx->hd_on) e = hd_stage_first(ctx, qs, s);
+        if (e != cudaSuccess) return e;
+        e = launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, A, qs, heating, qo, s);
+        if (e != cudaSuccess) return e;
+        if (ctx->hd_on) e = hd_stage_second(ctx, kRK3[st][2] * dt, qo, s);
         if (e != cudaSuccess) return e;
         e = launch_dss_classes(ctx, ctx->dss_int, qo, ctx->shell.FS, K_FUSED_DSS, s);
         if (e != cudaSuccess) return e;
@@ -769,7 +780,7 @@ static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const 
         }
         for (int step = 0; step < n_steps; ++step) {
             CKC(cudaGraphLaunch(ctx->graph, cs));
-            ctx->launches += 6;  // kernels replayed per step
+            ctx->launches += ctx->hd_on ? 18 : 6;  // kernels replayed per step
         }
         if (cs != s) {
             CKC(cudaEventRecord(ctx->gev1, cs));
@@ -868,7 +879,8 @@ extern "C" const char *numa_kernel_name(int32_t kernel_id)
 {
     static const char *names[K_COUNT] = {"k_rhs (volume)", "k_dss", "k_sources", "k_rk",
                                          "k_stage_volume (fused)", "k_stage_dss (fused)",
-                                         "k_shell_layout (natural <-> block-shell)"};
+                                         "k_shell_layout (natural <-> block-shell)",
+                                         "k_hd_lap (hyper-diffusion)", "k_hd_dss (hyper-diffusion)"};
     return (kernel_id >= 0 && kernel_id < K_COUNT) ? names[kernel_id] : "";
 }
 

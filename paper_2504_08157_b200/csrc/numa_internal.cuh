@@ -21,10 +21,13 @@ struct LglTables {
 };
 
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
-enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_COUNT = 7 };
+enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_HD = 7, K_HD_DSS = 8, K_COUNT = 9 };
 
 #ifndef NUMA_DSS_CHUNK
-#define NUMA_DSS_CHUNK 2048    // local nodes per DSS locality chunk (measured best of 256..2 M on cfg3)
+#define NUMA_DSS_CHUNK 2048    // positions per DSS locality chunk at N <= 4
+#endif
+#ifndef NUMA_DSS_CHUNK_HI
+#define NUMA_DSS_CHUNK_HI 32768 // ... at N >= 5 (numa_api.cu, dss_chunk)
 #endif
 #ifndef NUMA_DSS_THREADS
 #define NUMA_DSS_THREADS 64    // shared nodes per thread block of the DSS kernel
@@ -98,6 +101,9 @@ struct numa_ctx {
     uint8_t *face_bc;     // [Ne][8] (padded to 8 bytes per element)
     int32_t *d_flags;     // [4] device error flags
     int has_walls;
+    // tensor hyper-diffusion (numa_hd_init): tau[6][FS] block-shell and two 4-field work buffers
+    double *hd_tau = nullptr, *hd_buf = nullptr, *hd_buf2 = nullptr;
+    bool hd_on = false;
     bool attr_rhs = false, attr_stage = false;  // dynamic-shared-memory attribute set on this device
     int64_t launches;
     std::string err;
@@ -154,7 +160,11 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
                                 cudaStream_t s);
 // in-place DSS of r[5][stride] over one list set (kernel_id = profiling slot)
 cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_t stride,
-                               int kernel_id, cudaStream_t s);
+                               int kernel_id, cudaStream_t s, int nf = 5);
+// hyper-diffusion inside a fused stage (numa_hd.cu): h1 = DSS(omega L(qs[1..4])) before the volume
+// kernel; qout[1..4] += -b_dt P(omega L(h1)) after it (block-shell arrays)
+cudaError_t hd_stage_first(numa_ctx *c, const double *qs, cudaStream_t s);
+cudaError_t hd_stage_second(numa_ctx *c, double b_dt, double *qout, cudaStream_t s);
 // natural [nf][NL] <-> block-shell [nf][shell.FS]
 cudaError_t launch_to_shell(numa_ctx *c, const double *q_nat, double *q_int, int nf, cudaStream_t s);
 cudaError_t launch_from_shell(numa_ctx *c, const double *q_int, double *q_nat, int nf, cudaStream_t s);

@@ -223,8 +223,8 @@ k_ri_bins(const int32_t *__restrict__ chunk, const int32_t *__restrict__ uidx,
         if (!valid) continue;
         const double rx = xy[p] - xc, ry = xy[NL + p] - yc;
         const double r = sqrt(rx * rx + ry * ry);
-        if (!(r > 0.0) || !(r < r_max)) continue;
-        const double erx = rx / r, ery = ry / r;
+        if (!(r < r_max)) continue;
+        const double erx = (r > 0.0) ? rx / r : 0.0, ery = (r > 0.0) ? ry / r : 0.0;   // r = 0: no radial direction (Q29)
         const double ur = u * erx + v * ery;               // u . e_r (e_r has no z-component)
         const double t0 = u - ur * erx, t1 = v - ur * ery;   // w - (u . e_z) = 0: e_z removes the vertical part
         const double ut = sqrt(t0 * t0 + t1 * t1);

@@ -21,6 +21,9 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
 #define NUMA_SHELL_MAXRUN 16
 #endif
 static const int kMaxRun = NUMA_SHELL_MAXRUN;
+#ifndef NUMA_SHELL_ITERS
+#define NUMA_SHELL_ITERS 8
+#endif
 
 void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
                           std::vector<uint32_t> &tab)
@@ -88,13 +91,22 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
         }
         return c;
     };
+    // the quantity that matters: wavefronts of a thread-per-position 8-byte access, i.e. per
+    // half-warp the largest number of nodes in one bank, after the lanes have been dealt as below
+    auto wavefronts_ideal = [&]() {
+        for (int g = 0; g < ng; ++g)
+            if (group_cost(g) > 0) return false;
+        return true;
+    };
     uint64_t rng = 0x9E3779B97F4A7C15ull;
     auto rnd = [&]() { rng = rng * 6364136223846793005ull + 1442695040888963407ull; return (uint32_t)(rng >> 33); };
     flatten();
     int cur = 0;
     for (int g = 0; g < ng; ++g) cur += (gc[g] = group_cost(g));
     const int nblk = (int)blocks.size();
-    const long iters = 400000L + 4000L * nb;
+    // measured (pointwise wavefronts over the ideal two per request): 1.00 at N <= 5, 1.0-1.05 at
+    // N = 6 and 8; N = 7 (no pad positions, 16 nodes of every 8-byte bank pair) stays near 1.2
+    const long iters = (nb > 128 ? NUMA_SHELL_ITERS : 1) * (400000L + 4000L * nb);
     auto accept_step = [&](int delta, long it) {
         if (delta <= 0) return true;
         // accept an uphill step of d with probability 2^(-d / T), T falling linearly
@@ -103,11 +115,45 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
         return (rnd() & 0xffff) < (uint32_t)(pr * 65536.0);
     };
     for (long it = 0; it < iters && cur > 0; ++it) {
-        if ((rnd() & 31) == 0) {
-            // swap two whole blocks: every group between them changes
+        if ((it & 65535) == 0 && wavefronts_ideal()) break;
+        const uint32_t mv = rnd() & 31;
+        if (mv < 8) {
+            // swap two whole blocks (mostly two of equal length: cheap); a general swap moves
+            // every group between them
             int a = (int)(rnd() % nblk), b = (int)(rnd() % nblk);
+            if (mv >= 4) {
+                for (int tries = 0; tries < 4 && blocks[a].size() != blocks[b].size(); ++tries) b = (int)(rnd() % nblk);
+                if (blocks[a].size() != blocks[b].size()) continue;
+            }
             if (a == b) continue;
             if (a > b) std::swap(a, b);
+            if (blocks[a].size() == blocks[b].size()) {
+                // equal lengths: the other blocks stay where they are, only the groups under the
+                // two blocks change
+                const int L = (int)blocks[a].size();
+                int gs[8], ng2 = 0;
+                auto add_groups = [&](int s0) {
+                    for (int g = s0 / GW; g <= (s0 + L - 1) / GW; ++g) {
+                        bool seen = false;
+                        for (int q = 0; q < ng2; ++q) seen |= (gs[q] == g);
+                        if (!seen && ng2 < 8) gs[ng2++] = g;
+                    }
+                };
+                add_groups(start[a]); add_groups(start[b]);
+                int old = 0;
+                for (int q = 0; q < ng2; ++q) old += gc[gs[q]];
+                for (int t = 0; t < L; ++t) std::swap(seq[start[a] + t], seq[start[b] + t]);
+                int nw = 0, cs[8];
+                for (int q = 0; q < ng2; ++q) nw += (cs[q] = group_cost(gs[q]));
+                if (accept_step(nw - old, it)) {
+                    std::swap(blocks[a], blocks[b]);
+                    for (int q = 0; q < ng2; ++q) gc[gs[q]] = cs[q];
+                    cur += nw - old;
+                } else {
+                    for (int t = 0; t < L; ++t) std::swap(seq[start[a] + t], seq[start[b] + t]);
+                }
+                continue;
+            }
             const int lo = start[a] / GW;
             const int hi = (start[b] + (int)blocks[b].size() - 1) / GW;
             int old = 0;

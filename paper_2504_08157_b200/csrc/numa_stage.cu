@@ -106,7 +106,7 @@ struct StageShape {
     // PFS: the same 17 inputs are prefetched with cp.async into shared memory instead (no
     // registers held across phase B); used where one block per SM leaves the room (N = 6, 7).
 #ifndef STAGE_PFS_MASK
-#define STAGE_PFS_MASK 0x100  /* bit N set = use it (measured: pays at N = 8 only) */
+#define STAGE_PFS_MASK 0x000  /* bit N set = use it (with the L2 prefetch it no longer pays: N = 8 1.92 -> 1.79 ms without) */
 #endif
     static constexpr bool PFS = !PREFETCH && ((STAGE_PFS_MASK >> N) & 1);
     // PFS_ALL: all 17 inputs (met[9], omega, q0[5], heat, beta); otherwise only met and omega
@@ -283,6 +283,22 @@ __device__ __forceinline__ NodeIx node_ix(const uint32_t *__restrict__ tab, int 
     return x;
 }
 
+// Global accesses of the volume kernel: every value is used once per block, so nothing is
+// gained by allocating it in L1 (STAGE_LDMODE 0 = ld.global.nc / default stores, 1 = .cg, 2 = .cs)
+#ifndef STAGE_LDMODE
+#define STAGE_LDMODE 1
+#endif
+#if STAGE_LDMODE == 1
+#define VLD(p) __ldcg(p)
+#define VST(p, v) __stcg(p, v)
+#elif STAGE_LDMODE == 2
+#define VLD(p) __ldcs(p)
+#define VST(p, v) __stcs(p, v)
+#else
+#define VLD(p) __ldg(p)
+#define VST(p, v) (*(p) = (v))
+#endif
+
 template <int N>
 __global__ void __launch_bounds__(StageShape<N>::THREADS, StageShape<N>::MIN_BLOCKS)
 k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglTables tab)
@@ -362,21 +378,21 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
             }
         }
 #pragma unroll
-        for (int c = 0; c < 5; ++c) qv[rr][c] = A.qs[c * NL + p];
+        for (int c = 0; c < 5; ++c) qv[rr][c] = VLD(A.qs + c * NL + p);
         if constexpr (SH::PREFETCH) {
 #pragma unroll
-            for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
-            om = __ldg(A.omega + p);
+            for (int c = 0; c < 9; ++c) m[c] = VLD(A.met + c * NL + p);
+            om = VLD(A.omega + p);
             if (!same) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+                for (int c = 0; c < 5; ++c) q0v[c] = VLD(A.q0 + c * NL + p);
             }
-            if (A.heat) heat = __ldg(A.heat + p);
-            if (A.beta) beta = __ldg(A.beta + p);
+            if (A.heat) heat = VLD(A.heat + p);
+            if (A.beta) beta = VLD(A.beta + p);
         }
-        rho0[rr] = __ldg(A.ref3 + p);
-        const double th0 = __ldg(A.ref3 + NL + p), p0 = __ldg(A.ref3 + 2 * NL + p);
-        const double th0e = __ldg(A.ref3 + NL + rec + A.first_pos[x.le]);  // theta0 at the element's first node (Q7)
+        rho0[rr] = VLD(A.ref3 + p);
+        const double th0 = VLD(A.ref3 + NL + p), p0 = VLD(A.ref3 + 2 * NL + p);
+        const double th0e = VLD(A.ref3 + NL + rec + A.first_pos[x.le]);  // theta0 at the element's first node (Q7)
         const double xx = (qv[rr][0] * th0 + qv[rr][4] * rho0[rr] + qv[rr][0] * qv[rr][4]) / (rho0[rr] * th0);
         const double rho = rho0[rr] + qv[rr][0];
         sW[0 * FS + sp] = p0 * eos_ratio(xx, A.gamma, A.eos);
@@ -463,21 +479,21 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
         } else {
             if (!same) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+                for (int c = 0; c < 5; ++c) q0v[c] = VLD(A.q0 + c * NL + p);
             }
-            heat = A.heat ? __ldg(A.heat + p) : 0.0;
-            beta = A.beta ? __ldg(A.beta + p) : 0.0;
+            heat = A.heat ? VLD(A.heat + p) : 0.0;
+            beta = A.beta ? VLD(A.beta + p) : 0.0;
         }
     } else if constexpr (!SH::PREFETCH) {
 #pragma unroll
-        for (int c = 0; c < 9; ++c) m[c] = __ldg(A.met + c * NL + p);
-        om = __ldg(A.omega + p);
+        for (int c = 0; c < 9; ++c) m[c] = VLD(A.met + c * NL + p);
+        om = VLD(A.omega + p);
         if (!same) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
+            for (int c = 0; c < 5; ++c) q0v[c] = VLD(A.q0 + c * NL + p);
         }
-        heat = A.heat ? __ldg(A.heat + p) : 0.0;
-        beta = A.beta ? __ldg(A.beta + p) : 0.0;
+        heat = A.heat ? VLD(A.heat + p) : 0.0;
+        beta = A.beta ? VLD(A.beta + p) : 0.0;
     }
     const double rhop = qv[rr][0], u = qv[rr][1], v = qv[rr][2], w = qv[rr][3];
     const double irho = 1.0 / (rho0[rr] + rhop);
@@ -533,11 +549,11 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     if (same) {
         const double a01 = A.a0 + A.a1;
 #pragma unroll
-        for (int c = 0; c < 5; ++c) qop[c * NL] = om * (a01 * qv[rr][c]) + A.b_dt * r[c];
+        for (int c = 0; c < 5; ++c) VST(qop + c * NL, om * (a01 * qv[rr][c]) + A.b_dt * r[c]);
     } else {
 #pragma unroll
         for (int c = 0; c < 5; ++c)
-            qop[c * NL] = om * (A.a0 * q0v[c] + A.a1 * qv[rr][c]) + A.b_dt * r[c];
+            VST(qop + c * NL, om * (A.a0 * q0v[c] + A.a1 * qv[rr][c]) + A.b_dt * r[c]);
     }
     }  // rr
 }
@@ -818,9 +834,6 @@ k_stage_volume_p(const __grid_constant__ StageArgs A, const __grid_constant__ Lg
 // (idx[a*n + t]) so that the index loads coalesce and carry no dependent chain; all 5*C
 // values are loaded before the first store.  Sum in ascending local index.
 // ---------------------------------------------------------------------------------------
-#ifndef NUMA_DSS_FPT
-#define NUMA_DSS_FPT 5   // fields per thread: 1 (block = nodes x 5 fields) or 5
-#endif
 
 // the copies are touched once per launch by this SM: keep them out of L1 (ld/st .cg)
 #if !defined(NUMA_DSS_CA) && !defined(NUMA_DSS_CS)
@@ -856,20 +869,20 @@ __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__
     }
 }
 
-// block = (NUMA_DSS_THREADS shared nodes) x (5 / NUMA_DSS_FPT field groups)
+// block = NUMA_DSS_THREADS shared nodes, F fields per thread (5: the state; 4: hyper-diffusion)
 #ifndef NUMA_DSS_MINB
 #define NUMA_DSS_MINB 10  /* 96 registers; measured: neither more (12-20) nor fewer (1) resident blocks is faster */
 #endif
-__global__ void __launch_bounds__(NUMA_DSS_THREADS * (5 / NUMA_DSS_FPT), NUMA_DSS_MINB)
+template <int F>
+__global__ void __launch_bounds__(NUMA_DSS_THREADS, NUMA_DSS_MINB)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
             const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
             const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL)
 {
-    constexpr int F = NUMA_DSS_FPT;
     const DssSeg sg = segs[blkmap[blockIdx.x]];
     const int t = (blockIdx.x - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
     if (t >= sg.n) return;
-    double *rm = r + (int64_t)threadIdx.y * F * NL;
+    double *rm = r;
     if (sg.cls == 0) {
         dss_node<2, F>(rm, idx + sg.idx_base, sg.n, t, NL);
     } else if (sg.cls == 1) {
@@ -998,12 +1011,18 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
 }
 
 cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_t stride,
-                               int kernel_id, cudaStream_t s)
+                               int kernel_id, cudaStream_t s, int nf)
 {
     if (L.blocks == 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
-    k_stage_dss<<<(unsigned)L.blocks, dim3(NUMA_DSS_THREADS, 5 / NUMA_DSS_FPT), 0, s>>>(
-        r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start, L.copies, stride);
+    if (nf == 5)
+        k_stage_dss<5><<<(unsigned)L.blocks, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
+                                                                      L.copies, stride);
+    else if (nf == 4)
+        k_stage_dss<4><<<(unsigned)L.blocks, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
+                                                                      L.copies, stride);
+    else
+        return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 

@@ -32,8 +32,21 @@ def _compare(wl, q, r_max, n_strips=50, g=None):
     assert np.abs(cg - o["centroid"])[valid].max(initial=0.0) <= TOL * L
     assert (count == o["count"]).all()                      # bin decisions: bit-exact
     scale = max(o["umax_h"], 1e-300)
-    assert np.abs(ubar - o["ubar"]).max() <= TOL * scale
-    assert abs(sc[0] - o["u_ri"]) <= TOL * scale
+    # Eq. 21 is ill-conditioned at the centroid itself: a point with r ~ 1e-16 L has an e_r that is
+    # pure rounding, and its u_theta may be anything in [0, |u_h|].  Such a point (at most one per
+    # level, in strip 0) widens the bound of its strip mean by |u_h| / count.
+    flat = mesh.intma_cg.reshape(-1)
+    _, first = np.unique(flat, return_index=True)
+    px, py = mesh.xyz[0].reshape(-1)[first], mesh.xyz[1].reshape(-1)[first]
+    pl = lev.reshape(-1)[first]
+    uh = np.hypot(q[1].reshape(-1)[first], q[2].reshape(-1)[first])
+    r = np.hypot(px - o["centroid"][pl, 0], py - o["centroid"][pl, 1])
+    slack = np.zeros_like(ubar)
+    for t in np.nonzero(r < 1e-6 * L)[0]:
+        slack[pl[t], 0] += uh[t] / max(o["count"][pl[t], 0], 1)
+    assert (np.abs(ubar - o["ubar"]) <= TOL * scale + slack).all()
+    assert slack.max() <= 1e-6 * scale          # ... and it is a tiny correction, not a loophole
+    assert abs(sc[0] - o["u_ri"]) <= TOL * scale + slack.max()
     assert abs(sc[1] - o["umax_h"]) <= 4e-16 * scale          # the GPU may contract u*u + v*v into an FMA
     return o, g
 
