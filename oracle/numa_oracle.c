@@ -641,3 +641,72 @@ void orc_hd_laplacian(int N, long Ne, int nf, const double *met, const double *t
         free(F);
     }
 }
+
+/* ------------------------------------------------------------------------------------
+ * NEXT-3  Linear operator of the IMEX splitting (Section 2.3, Eq. 13):
+ *     dq/dt = [S(q) - L(q)] + L(q),
+ * "the linear operator L(q) represent[s] fast waves, such as acoustic and gravity waves".
+ * The paper does not print L (it cites Giraldo et al. 2013); reading Q34 of DESIGN.md: L is the
+ * linearisation (Jacobian) of the S of Eq. 1 about the hydrostatic reference state q = 0,
+ *     L_rho   = - div( rho0 u )
+ *     L_u     = - grad p'_L / rho0 - (rho'/rho0) g k,
+ *               p'_L = gamma p0 ( rho'/rho0 + theta'/theta0 )   (Eq. 3 linearised; p0 = EOS(rho0,theta0))
+ *     L_theta = - u . grad theta0
+ * evaluated element-locally exactly as orc_tendency evaluates S (Alg. 2 derivatives + chain
+ * rule, Q2; grad theta0 relative to the element's first node, Q7).  Pinned as the directional
+ * derivative of orc_tendency: L(v) = lim S(eps v)/eps (tests/test_oracle_imex.py).
+ * ---------------------------------------------------------------------------------- */
+void orc_linear_tendency(int N, long Ne, const double *par, const double *q, const double *ref,
+                         const double *met, double *Lq)
+{
+    int Nq = N + 1;
+    long Mn = (long)Nq * Nq * Nq, NL = Ne * Mn;
+    double g = par[0], p_a = par[1], R = par[2], c_p = par[3], c_v = par[4];
+    double gamma = c_p / c_v;
+    double xi[64], w[64], D[64 * 64];
+    orc_lgl(N, xi, w);
+    orc_dmat(N, xi, D);
+#pragma omp parallel
+    {
+        double *wk = (double *)malloc(sizeof(double) * 5 * Mn);
+        double *pl = wk, *th0 = wk + Mn, *Fx = wk + 2 * Mn, *Fy = wk + 3 * Mn, *Fz = wk + 4 * Mn;
+#pragma omp for schedule(static)
+        for (long e = 0; e < Ne; ++e) {
+            long b = e * Mn;
+            for (long n = 0; n < Mn; ++n) {
+                double rho0 = ref[0 * NL + b + n], theta0 = ref[1 * NL + b + n];
+                double p0 = p_a * pow(rho0 * R * theta0 / p_a, gamma);
+                pl[n] = gamma * p0 * (q[0 * NL + b + n] / rho0 + q[4 * NL + b + n] / theta0);
+                th0[n] = theta0 - ref[1 * NL + b];
+                Fx[n] = rho0 * q[1 * NL + b + n];
+                Fy[n] = rho0 * q[2 * NL + b + n];
+                Fz[n] = rho0 * q[3 * NL + b + n];
+            }
+            for (int k = 0; k < Nq; ++k)
+                for (int j = 0; j < Nq; ++j)
+                    for (int i = 0; i < Nq; ++i) {
+                        long p = b + NODE(i, j, k);
+                        double m[9];
+                        for (int c = 0; c < 9; ++c) m[c] = met[c * NL + p];
+                        double fx, fe, fz, gp[3], gt[3], div = 0.0;
+                        ref_derivs(Nq, D, pl, i, j, k, &fx, &fe, &fz);
+                        for (int c = 0; c < 3; ++c) gp[c] = fx * m[0 + c] + fe * m[3 + c] + fz * m[6 + c];
+                        ref_derivs(Nq, D, th0, i, j, k, &fx, &fe, &fz);
+                        for (int c = 0; c < 3; ++c) gt[c] = fx * m[0 + c] + fe * m[3 + c] + fz * m[6 + c];
+                        const double *F[3] = {Fx, Fy, Fz};
+                        for (int c = 0; c < 3; ++c) {
+                            ref_derivs(Nq, D, F[c], i, j, k, &fx, &fe, &fz);
+                            div += fx * m[0 + c] + fe * m[3 + c] + fz * m[6 + c];
+                        }
+                        double rho0 = ref[0 * NL + p];
+                        double u = q[1 * NL + p], v = q[2 * NL + p], wv = q[3 * NL + p];
+                        Lq[0 * NL + p] = -div;
+                        Lq[1 * NL + p] = -gp[0] / rho0;
+                        Lq[2 * NL + p] = -gp[1] / rho0;
+                        Lq[3 * NL + p] = -gp[2] / rho0 - (q[0 * NL + p] / rho0) * g;
+                        Lq[4 * NL + p] = -(u * gt[0] + v * gt[1] + wv * gt[2]);
+                    }
+        }
+        free(wk);
+    }
+}

@@ -23,6 +23,18 @@ _LIB = os.path.join(_HERE, "libnuma_oracle.so")
 # SSP-RK3 (Shu-Osher) as (a0, a1, b):  q_out = a0 q0 + a1 qs + b dt L(qs)
 SSP_RK3 = ((1.0, 0.0, 1.0), (0.75, 0.25, 0.25), (1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0))
 
+# ARK2 of Giraldo, Kelly & Constantinescu 2013 ("the second-order additive
+# Runge-Kutta (ARK2) scheme proposed in (Giraldo et al. 2013)"; the paper does not print the
+# tableau: reading Q35 of DESIGN.md).  Three stages, gamma = 1 - 1/sqrt(2); explicit A, implicit
+# At (singly diagonally implicit, first stage explicit), b shared.  Pinned by the order conditions
+# and by measured second-order convergence (tests/test_oracle_imex.py).
+_G = 1.0 - 1.0 / np.sqrt(2.0)
+_A32 = (3.0 + 2.0 * np.sqrt(2.0)) / 6.0
+_B = 1.0 / (2.0 * np.sqrt(2.0))
+ARK2_A = ((0.0, 0.0, 0.0), (2.0 * _G, 0.0, 0.0), (1.0 - _A32, _A32, 0.0))
+ARK2_AT = ((0.0, 0.0, 0.0), (_G, _G, 0.0), (_B, _B, _G))
+ARK2_B = (_B, _B, _G)
+
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain -O2, OpenMP over elements, no FP contraction)."""
@@ -62,6 +74,7 @@ def lib():
         L.orc_walls.argtypes = [C.c_long, C.c_long, C.POINTER(C.c_int64), _dp, _dp]
         L.orc_rk_stage.argtypes = [C.c_long, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp]
         L.orc_hd_laplacian.argtypes = [C.c_int, C.c_long, C.c_int, _dp, _dp, _dp, _dp]
+        L.orc_linear_tendency.argtypes = [C.c_int, C.c_long, _dp, _dp, _dp, _dp, _dp]
         _ip = C.POINTER(C.c_int32)
         L.orc_ri_area.argtypes = [C.c_int, C.c_long, _dp, _dp]
         L.orc_ri_velocity.argtypes = [C.c_long, C.c_long, _ip, _ip, C.c_int, C.c_int, C.c_double,
@@ -158,6 +171,67 @@ def rk_stage(a0, a1, b_dt, q0, qs, r, out=None):
         out = np.empty_like(q0)
     lib().orc_rk_stage(q0.size, a0, a1, b_dt, _p(q0), _p(qs), _p(r), _p(out))
     return out
+
+
+def linear_tendency(N, par, q, ref, met):
+    """Element-local linear operator L_loc(q) of the IMEX splitting (Eq. 13; reading Q34)."""
+    q = _f64(q)
+    out = np.empty_like(q)
+    lib().orc_linear_tendency(N, q.shape[1], _p(_f64(par)), _p(q), _p(_f64(ref)), _p(met), _p(out))
+    return out
+
+
+def gmres(apply_A, b, x0, dot, tol, m, max_restarts):
+    """Restarted GMRES(m) of Saad & Schultz 1986, written out: Arnoldi with
+    modified Gram-Schmidt, Givens rotations on the Hessenberg matrix, no preconditioner.
+    Stops when ||r|| <= tol ||b|| (residual norm from the rotated right-hand side).
+    Returns (x, inner iterations, relative residual estimate)."""
+    x = x0.copy()
+    bnorm = np.sqrt(dot(b, b))
+    if bnorm == 0.0:
+        return np.zeros_like(b), 0, 0.0
+    its = 0
+    rel = np.inf
+    for _ in range(max_restarts + 1):
+        r = b - apply_A(x)
+        beta = np.sqrt(dot(r, r))
+        rel = beta / bnorm
+        if rel <= tol:
+            break
+        V = [r / beta]
+        H = np.zeros((m + 1, m))
+        cs = np.zeros(m); sn = np.zeros(m)
+        g = np.zeros(m + 1); g[0] = beta
+        k_used = 0
+        for k in range(m):
+            w = apply_A(V[k])
+            for i in range(k + 1):
+                H[i, k] = dot(w, V[i])
+                w = w - H[i, k] * V[i]
+            hn = np.sqrt(dot(w, w))
+            H[k + 1, k] = hn
+            for i in range(k):
+                t = cs[i] * H[i, k] + sn[i] * H[i + 1, k]
+                H[i + 1, k] = -sn[i] * H[i, k] + cs[i] * H[i + 1, k]
+                H[i, k] = t
+            d = np.hypot(H[k, k], H[k + 1, k])
+            cs[k] = H[k, k] / d; sn[k] = H[k + 1, k] / d
+            H[k, k] = d; H[k + 1, k] = 0.0
+            g[k + 1] = -sn[k] * g[k]; g[k] = cs[k] * g[k]
+            its += 1
+            k_used = k + 1
+            rel = abs(g[k + 1]) / bnorm
+            if rel <= tol or d == 0.0:
+                break
+            V.append(w / hn)
+        y = np.zeros(k_used)
+        for i in range(k_used - 1, -1, -1):
+            y[i] = (g[i] - H[i, i + 1:k_used] @ y[i + 1:]) / H[i, i]
+        for i in range(k_used):
+            x = x + y[i] * V[i]
+        if rel <= tol:
+            break
+    return x, its, rel
 
 
 def hd_tau(met, c, dt):
@@ -285,6 +359,49 @@ class Oracle:
         self.dss(r)
         self.apply_sources(q, heat, r)
         return r
+
+    # --- NEXT-3: IMEX (Eq. 13), ARK2 + matrix-free GMRES (L127-L137) --------------------------
+    def linear(self, q):
+        """L_h(q) = walls(DSS(omega * L_loc(q))): the linear operator assembled like S (Eq. 11-12),
+        with the no-flux projection; no sources (they stay in the explicit part)."""
+        r = weight(self.omega, linear_tendency(self.N, self.par, q, self.ref, self.met))
+        self.dss(r)
+        walls(self.wall_node, self.wall_normal, r)
+        return r
+
+    def dot(self, a, b):
+        """Euclidean inner product over the unique global nodes (each local copy weighted by
+        1 / multiplicity), all five fields: the inner product of the GMRES (reading Q36)."""
+        if not hasattr(self, "_inv_mult"):
+            cnt = np.bincount(self.intma_cg.reshape(-1), minlength=self.n_global)
+            self._inv_mult = (1.0 / cnt[self.intma_cg]).reshape(1, *self.intma_cg.shape)
+        return float(np.sum(self._inv_mult * a * b))
+
+    def step_ark2(self, q, dt, heat=None, tol=1e-10, m=20, max_restarts=10, stats=None):
+        """One IMEX ARK2 step (Eq. 13): explicit part N = S - L, implicit part L, stages
+            Q_i = q + dt sum_{j<i} (a_ij N(Q_j) + at_ij L(Q_j)) + dt at_ii L(Q_i),
+        the linear systems (I - dt at_ii L) Q_i = R_i solved by GMRES(m) from the initial guess R_i;
+        q_new = q + dt sum b_i S(Q_i)."""
+        q = _f64(q)
+        Nq, Lq, Sq = [], [], []
+        for i in range(3):
+            R = q.copy()
+            for j in range(i):
+                R = R + dt * (ARK2_A[i][j] * Nq[j] + ARK2_AT[i][j] * Lq[j])
+            aii = ARK2_AT[i][i]
+            if aii == 0.0:
+                Q = R
+            else:
+                Q, its, rel = gmres(lambda x: x - dt * aii * self.linear(x), R, R, self.dot, tol, m, max_restarts)
+                if stats is not None:
+                    stats.append((its, rel))
+            S = self.rhs(Q, heat)
+            L = self.linear(Q)
+            Sq.append(S); Lq.append(L); Nq.append(S - L)
+        out = q.copy()
+        for i in range(3):
+            out = out + dt * ARK2_B[i] * Sq[i]
+        return out
 
     def step_rk3(self, q, dt, heat=None):
         """A11: one SSP-RK3 step (Q11)."""

@@ -22,7 +22,7 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
 #endif
 static const int kMaxRun = NUMA_SHELL_MAXRUN;
 #ifndef NUMA_SHELL_ITERS
-#define NUMA_SHELL_ITERS 8
+#define NUMA_SHELL_ITERS 2
 #endif
 
 void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,

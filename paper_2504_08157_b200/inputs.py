@@ -455,9 +455,16 @@ CFG4_NXY = {3: 158, 4: 113, 5: 86, 6: 68, 7: 56, 8: 47}
 CFG4_DT = {3: 0.15, 4: 0.10, 5: 0.07, 6: 0.055, 7: 0.043, 8: 0.034}
 
 
-def make_workload(config: int, N: Optional[int] = None, scale: float = 1.0) -> Workload:
+# config 4's two literal examples (BASELINE.json: "N=4: 200x200x20 elements; N=7: 125x125x16"), which
+# contradict its "~32M local nodes" (100 M and 128 M nodes; reading Q14): run as extra rows
+CFG4_LITERAL = {4: (200, 20), 7: (125, 16)}
+
+
+def make_workload(config: int, N: Optional[int] = None, scale: float = 1.0,
+                  literal: bool = False) -> Workload:
     """Build BASELINE.json config 1..5.  `scale` < 1 shrinks the horizontal element counts
-    (used by tests and by the bounded CPU-baseline sample); the physics is unchanged."""
+    (used by tests and by the bounded CPU-baseline sample); the physics is unchanged.
+    literal=True (config 4, N = 4 or 7): the element counts BASELINE.json gives as examples."""
     if config == 1:
         N = 4 if N is None else N
         mesh = box_mesh(N, 4, 4, 4, (1000.0, 1000.0, 1000.0), perturb=0.05,
@@ -483,6 +490,11 @@ def make_workload(config: int, N: Optional[int] = None, scale: float = 1.0) -> W
                             dt=0.1, n_steps=200)
     if config == 4:
         N = 4 if N is None else N
+        if literal:
+            nxy, nz = CFG4_LITERAL[N]
+            nx = max(2, int(round(nxy * scale)))
+            return _tc_workload(4, "cfg4_literal_%dx%dx%d_N%d" % (nx, nx, nz, N), N, nx, nx, nz,
+                                dt=CFG4_DT[N], n_steps=20)
         nx = max(2, int(round(CFG4_NXY[N] * scale)))
         return _tc_workload(4, "cfg4_sweep_%dx%dx20_N%d" % (nx, nx, N), N, nx, nx, 20,
                             dt=CFG4_DT[N], n_steps=20)

@@ -474,12 +474,14 @@ def test_full_size_cfg3_in_the_bench_configuration():
         assert np.array_equal(f, f[first[cg]])
 
 
-def test_full_size_cfg4_N7_sweep_point():
-    """Config 4 at N=7 in full (56x56x20 elements, 32.1 M local nodes: the element size of
-    config 5 and the launch configuration of the high-order kernels): one fused SSP-RK3 step
-    against the oracle, element by element."""
-    wl = inputs.make_workload(4, N=7)
-    assert wl.mesh.n_local == 32_112_640
+@pytest.mark.parametrize("N,n_local", [(3, 31_953_920), (4, 31_922_500), (5, 31_950_720), (6, 31_720_640),
+                                       (7, 32_112_640), (8, 32_207_220)])
+def test_full_size_cfg4_sweep_point(N, n_local):
+    """Config 4 in full at every order of the sweep (~32 M local nodes, the launch configuration
+    bench.py times; N = 7 is also the element size of config 5): one fused SSP-RK3 step against
+    the oracle, element by element."""
+    wl = inputs.make_workload(4, N=N)
+    assert wl.mesh.n_local == n_local
     o, g = _pair(wl)
     hd = g.state(wl.heating)
     qd = g.state(wl.q)
@@ -492,9 +494,11 @@ def test_full_size_cfg4_N7_sweep_point():
     vel = np.sqrt(sum(np.linalg.norm(q[m]) ** 2 for m in (1, 2, 3)))
     den = [np.linalg.norm(q[0]), vel, vel, vel, np.linalg.norm(q[4])]
     e = np.array([np.linalg.norm(qg[m] - q[m]) / den[m] for m in range(5)])
-    record("FULL SIZE cfg4 N=7: state after 1 RK3 step (fused route)", [4, 7, 1.0], qg, q)
+    record("FULL SIZE cfg4 N=%d: state after 1 RK3 step (fused route)" % N, [4, N, 1.0], qg, q)
     assert np.all(e <= TOL_RHS * 3), e      # three stages, each within the per-call tolerance
     assert np.all(rel_l2(qg, q) <= TOL_100)  # and plainly per field within the 100-step bound
+    del o, g, qd, hd
+    torch.cuda.empty_cache()
 
 
 # ---------------------------------------------------------------------------------------
