@@ -215,6 +215,40 @@ numa_status numa_hd_init(numa_ctx *ctx, const double *c3, double dt_ref, void *h
 numa_status numa_hyperdiffusion(numa_ctx *ctx, const double *q, double *rhs, void *stream);
 
 /*
+ * IMEX time integration (Section 2.3, Eq. 13):
+ * dq/dt = [S(q) - L(q)] + L(q) with the fast acoustic / gravity waves in the linear operator L,
+ * integrated by the additive Runge-Kutta scheme ARK2 (L133) whose implicit stages are solved by
+ * matrix-free GMRES (L135).  The paper prints neither L nor the tableau; readings Q34-Q36:
+ *   - L = the Jacobian of the S of Eq. 1 at the reference state q = 0:
+ *       L_rho = -div(rho0 u);   L_u = -grad p'_L / rho0 - (rho'/rho0) g k,
+ *       p'_L = gamma p0 (rho'/rho0 + theta'/theta0);   L_theta = -u . grad theta0,
+ *     assembled like S, L_h = P(DSS(omega L_loc)), P the no-flux projection; heating, Coriolis
+ *     and the sponge stay in the explicit part;
+ *   - ARK2 of Giraldo, Kelly & Constantinescu 2013: 3 stages, gamma = 1 - 1/sqrt(2), explicit
+ *     a21 = 2 gamma, a32 = (3 + 2 sqrt(2))/6, a31 = 1 - a32; implicit rows (gamma, gamma, 0) and
+ *     b = (1/(2 sqrt 2), 1/(2 sqrt 2), gamma) (stiffly accurate), b shared by both parts;
+ *   - GMRES(m) of Saad & Schultz 1986: modified Gram-Schmidt, Givens rotations, no
+ *     preconditioner, initial guess = the stage's right-hand side, stop at ||r|| <= tol ||b||,
+ *     inner product = Euclidean over the unique global nodes.
+ *
+ * numa_imex_init (enqueue only): m = Krylov vectors per restart cycle (the paper: "fewer than 20");
+ *   imex_workspace (>= numa_imex_workspace_bytes(p, m), 256-byte aligned, caller-owned) holds the
+ *   (m + 13) state-sized work vectors.
+ * numa_linear_operator (enqueue only): Lq = L_h(q), both [5][Ne][Mn]; Lq must not alias q.
+ * numa_step_ark2 (SYNCHRONISES `stream`: every GMRES inner product is read back by the host):
+ *   n_steps ARK2 steps of size dt in place on q[5][Ne][Mn]; S is evaluated through the four-call
+ *   route.  gmres_iterations / max_rel_residual (host pointers, may be NULL) receive the total
+ *   number of Krylov iterations and the largest final relative residual of the implicit solves.
+ */
+size_t numa_imex_workspace_bytes(const numa_params *p, int32_t m);
+numa_status numa_imex_init(numa_ctx *ctx, int32_t m, void *imex_workspace, size_t workspace_bytes,
+                           void *stream);
+numa_status numa_linear_operator(numa_ctx *ctx, const double *q, double *Lq, void *stream);
+numa_status numa_step_ark2(numa_ctx *ctx, double *q, const double *heating, double dt, int32_t n_steps,
+                           double tol, int32_t max_restarts, int64_t *gmres_iterations,
+                           double *max_rel_residual, void *stream);
+
+/*
  * RI-velocity diagnostic (Eq. 18-22) on the device;
  * the paper computes it on the CPU after copying the state back (L172).  Readings Q25-Q29 of
  * DESIGN.md:

@@ -23,7 +23,8 @@ EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometr
            "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
            "numa_step_rk3_graph", "numa_step_rk3_host", "numa_copy_table", "numa_destroy",
            "numa_last_error", "numa_ri_workspace_bytes", "numa_ri_init", "numa_ri_velocity",
-           "numa_ri_destroy", "numa_hd_workspace_bytes", "numa_hd_init", "numa_hyperdiffusion"]
+           "numa_ri_destroy", "numa_hd_workspace_bytes", "numa_hd_init", "numa_hyperdiffusion",
+           "numa_imex_workspace_bytes", "numa_imex_init", "numa_linear_operator", "numa_step_ark2"]
 MEASURE_EXPORTS = ["numa_profile_enable", "numa_profile_read", "numa_kernel_name",
                    "numa_kernel_count", "numa_launch_count", "numa_measure_fp64_peak"]
 
@@ -69,6 +70,12 @@ def load_library(path: str | None = None):
     L.numa_step_rk3_graph.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
     L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
+    L.numa_imex_workspace_bytes.argtypes = [C.POINTER(NumaParams), C.c_int32]
+    L.numa_imex_workspace_bytes.restype = C.c_size_t
+    L.numa_imex_init.argtypes = [vp, C.c_int32, vp, C.c_size_t, vp]
+    L.numa_linear_operator.argtypes = [vp, dp, dp, vp]
+    L.numa_step_ark2.argtypes = [vp, dp, dp, C.c_double, C.c_int32, C.c_double, C.c_int32,
+                                 C.POINTER(C.c_int64), C.POINTER(C.c_double), vp]
     L.numa_hd_workspace_bytes.argtypes = [C.POINTER(NumaParams)]
     L.numa_hd_workspace_bytes.restype = C.c_size_t
     L.numa_hd_init.argtypes = [vp, C.POINTER(C.c_double), C.c_double, vp, C.c_size_t, vp]
@@ -97,7 +104,8 @@ def load_library(path: str | None = None):
     for f in ("numa_init_geometry", "numa_rhs", "numa_dss_or_flux", "numa_apply_sources",
               "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_graph", "numa_step_rk3_host",
               "numa_copy_table", "numa_ri_init", "numa_ri_velocity", "numa_ri_destroy",
-              "numa_hd_init", "numa_hyperdiffusion", "numa_destroy"):
+              "numa_hd_init", "numa_hyperdiffusion", "numa_imex_init", "numa_linear_operator",
+              "numa_step_ark2", "numa_destroy"):
         getattr(L, f).restype = C.c_int
     if path is None:
         _LIB = L
@@ -226,6 +234,26 @@ class Numa:
                                                 _ptr(d_q), _ptr(d_heating), _ptr(self.scratch()),
                                                 dt, n_steps, _stream()))
         return q_host
+
+    # -- IMEX: linear operator, ARK2 + GMRES (numa_imex_*, numa_step_ark2) ---------------------
+    def imex_init(self, m=20):
+        n = self.lib.numa_imex_workspace_bytes(C.byref(self.params), m)
+        if n == 0:
+            raise NumaError(1, "numa_imex_workspace_bytes: parameters out of range")
+        self._imex_ws = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._check(self.lib.numa_imex_init(self.ctx, m, _ptr(self._imex_ws), n, _stream()))
+
+    def linear_operator(self, q, out=None):
+        out = torch.empty_like(q) if out is None else out
+        self._check(self.lib.numa_linear_operator(self.ctx, _ptr(q), _ptr(out), _stream()))
+        return out
+
+    def step_ark2(self, q, dt, heating=None, n_steps=1, tol=1e-10, max_restarts=10):
+        """numa_step_ark2 -> (total GMRES iterations, largest final relative residual)."""
+        its = C.c_int64(0); rel = C.c_double(0.0)
+        self._check(self.lib.numa_step_ark2(self.ctx, _ptr(q), _ptr(heating), dt, n_steps, tol, max_restarts,
+                                            C.byref(its), C.byref(rel), _stream()))
+        return its.value, rel.value
 
     def hd_init(self, c3, dt_ref):
         """numa_hd_init: tensor hyper-diffusion (Eq. 14-16) on; c3 = (c_1, c_2, c_3)."""

@@ -104,6 +104,9 @@ struct numa_ctx {
     // tensor hyper-diffusion (numa_hd_init): tau[6][FS] block-shell and two 4-field work buffers
     double *hd_tau = nullptr, *hd_buf = nullptr, *hd_buf2 = nullptr;
     bool hd_on = false;
+    // IMEX (numa_imex_init): inv_mult[NL] followed by the Krylov and ARK work vectors
+    char *imex_ws = nullptr;
+    int imex_m = 0;
     bool attr_rhs = false, attr_stage = false;  // dynamic-shared-memory attribute set on this device
     int64_t launches;
     std::string err;

@@ -1,0 +1,70 @@
+"""GPU parity of the IMEX path (numa_linear_operator, numa_step_ark2; Eq. 13) against
+the CPU oracle: the linear operator per call at 1e-12; ARK2 steps, whose implicit stages both
+sides solve with the same GMRES(m) to a relative residual tol, at 100 tol (the two Krylov
+iterations differ by rounding, their solutions by at most the residual tolerance times the
+conditioning of I - dt gamma L, which is < 10 here)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as orc
+from paper_2504_08157_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("cfg,N,scale", [(1, 4, 1.0), (1, 2, 1.0), (2, 7, 0.2), (3, 4, 0.06), (4, 5, 0.05), (5, 7, 0.03), (4, 8, 0.05)])
+def test_linear_operator_matches_oracle(cfg, N, scale):
+    wl = inputs.make_workload(cfg, N=N, scale=scale)
+    o = orc.Oracle.from_workload(wl)
+    g = binding.Numa.from_workload(wl)
+    q = inputs.smooth_random_state(wl.mesh, wl.ref[0], wl.ref[1], seed=21)
+    Lo = o.linear(q)
+    Lg = g.linear_operator(g.state(q)).cpu().numpy()
+    for m in range(5):
+        err = np.linalg.norm(Lg[m] - Lo[m]) / np.linalg.norm(Lo[m])
+        assert err <= 1e-12, (m, err)
+
+
+@pytest.mark.parametrize("cfg,N,scale,dt,steps", [(1, 4, 1.0, 0.05, 3), (3, 4, 0.05, 0.5, 3), (2, 5, 0.2, 0.04, 2),
+                                                   (5, 7, 0.025, 0.5, 2)])
+def test_ark2_steps_match_oracle(cfg, N, scale, dt, steps):
+    """dt is several times the explicit limit of each mesh (config 3 / 5: the paper's 0.5 s, L296)."""
+    wl = inputs.make_workload(cfg, N=N, scale=scale)
+    o = orc.Oracle.from_workload(wl)
+    g = binding.Numa.from_workload(wl)
+    g.imex_init(20)
+    tol = 1e-11
+    stats = []
+    qo = wl.q
+    for _ in range(steps):
+        qo = o.step_ark2(qo, dt, wl.heating, tol=tol, m=20, max_restarts=20, stats=stats)
+    qd = g.state(wl.q)
+    heat = None if wl.heating is None else g.state(wl.heating)
+    its, rel = g.step_ark2(qd, dt, heat, steps, tol=tol, max_restarts=20)
+    qg = qd.cpu().numpy()
+    assert np.isfinite(qg).all() and rel <= tol
+    its_o = sum(i for i, _ in stats)
+    assert abs(its - its_o) <= max(2, its_o // 10), (its, its_o)     # same algorithm, same iteration counts
+    vel = np.sqrt(sum(np.linalg.norm(qo[m]) ** 2 for m in (1, 2, 3)))
+    den = [np.linalg.norm(qo[0]), vel, vel, vel, np.linalg.norm(qo[4])]
+    for m in range(5):
+        err = np.linalg.norm(qg[m] - qo[m]) / den[m]
+        assert err <= 100 * tol, (m, err)
+    # bitwise reproducible run to run
+    qd2 = g.state(wl.q)
+    g.step_ark2(qd2, dt, heat, steps, tol=tol, max_restarts=20)
+    assert torch.equal(qd, qd2)
+
+
+def test_imex_errors_are_status_codes():
+    wl = inputs.make_workload(1)
+    g = binding.Numa.from_workload(wl)
+    q = g.state(wl.q)
+    with pytest.raises(binding.NumaError):
+        g.step_ark2(q, 0.01)                       # before numa_imex_init
+    with pytest.raises(binding.NumaError):
+        g.imex_init(0)
+    g.imex_init(5)
+    with pytest.raises(binding.NumaError):
+        g.step_ark2(q, 0.01, tol=0.0)
