@@ -39,6 +39,8 @@ def parse_workload(name):
         return 4, -int(name[-1])     # negative N: BASELINE.json's literal element counts (Q14)
     if name.startswith("cfg4n"):
         return 4, int(name[5:])
+    if name == "table1":
+        return 0, 5                  # the paper's Table-1 grid (80x80x24, N=5; inputs.paper_table1_workload)
     if name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
         return int(name[3]), None
     raise SystemExit("unknown workload %r" % name)
@@ -64,6 +66,12 @@ def volume_alg_bytes(N, has_src):
 def dss_alg_bytes(N):
     """The DSS kernel's share of B_alg: face nodes of 5 fields read and written once."""
     return 2 * 8 * 5 * f_face(N)
+
+
+def hd_lap_alg_bytes():
+    """One application of omega div(tau grad .) to 4 fields: 4 in, 4 out (the second application also
+    reads the 4 it accumulates into: counted as +2 on average), grad xi (9), tau (6), omega (1)."""
+    return 8.0 * (4 + 4 + 2 + 9 + 6 + 1)
 
 
 def f_alg_flops(N):
@@ -263,10 +271,16 @@ def run_gpu(args):
     config, N_arg = parse_workload(args.workload)
     literal = N_arg is not None and N_arg < 0
     N_arg = -N_arg if literal else N_arg
-    wl = inputs.make_workload(config, N=N_arg, literal=literal)
+    wl = inputs.paper_table1_workload() if config == 0 else inputs.make_workload(config, N=N_arg, literal=literal)
+    if args.integrator == "ark2":
+        return run_gpu_ark2(args, wl, dev, rank, world)
     mesh = wl.mesh
     NL = mesh.n_local
     g = binding.Numa.from_workload(wl, device=str(dev))
+    if args.hyperdiffusion:
+        # tensor hyper-diffusion on (Eq. 14-16): coefficients that put dt * rho(H) near 1 on the
+        # config-3 element shapes (measured with the oracle, tests/test_gpu_hyperdiffusion.py)
+        g.hd_init((1.5e-5, 1.5e-5, 4.5e-5), wl.dt)
     q = g.state(wl.q)
     heat = None if wl.heating is None else g.state(wl.heating)
     g.scratch()
@@ -357,6 +371,10 @@ def run_gpu(args):
     has_src = wl.heating is not None
     N = mesh.N
     balg, falg = b_alg_bytes(N, has_src), f_alg_flops(N)
+    if args.hyperdiffusion:
+        # two Laplacian applications (12 + 36 contractions each on 4 fields) and one more 4-field DSS
+        balg += 2 * hd_lap_alg_bytes() + dss_alg_bytes(N) * 4.0 / 5.0
+        falg += 2 * (4 * 48 * 2.0 * (N + 1) + 4 * 60.0)
     stage_ms = ms / (3 * args.steps)
     hbm_achieved = balg * NL / (stage_ms * 1e-3) / 1e9             # GB/s, algorithmic
     fp64_achieved = falg * NL / (stage_ms * 1e-3) / 1e12           # TFLOP/s, algorithmic
@@ -413,6 +431,7 @@ def run_gpu(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl.name, "N": mesh.N, "elements": [mesh.nx, mesh.ny, mesh.nz],
                    "local_nodes": NL, "integrator": "SSP-RK3 (3 RHS + 3 stage updates per step)",
+                   "hyperdiffusion": bool(args.hyperdiffusion),
                    "dt": wl.dt, "multi_gpu": "replicas only" if world > 1 else "single",
                    "launch": "CUDA graph per step" if args.graph else "plain launches",
                    "l2": "inputs larger than L2" if 22 * NL * 8 > 4 * 126e6 else
@@ -435,6 +454,54 @@ def run_gpu(args):
         raise SystemExit("bench.py: the state is not finite after the timed steps; no value reported")
 
 
+def run_gpu_ark2(args, wl, dev, rank, world):
+    """--integrator ark2: the paper's own integrator (IMEX ARK2 + matrix-free GMRES, Eq. 13) through
+    numa_step_ark2.  Reported: ms per IMEX step (the quantity of the paper's Table 1), Krylov
+    iterations per step, and nodal operator applications (S or L) per second."""
+    import torch
+    from paper_2504_08157_b200 import binding
+    g = binding.Numa.from_workload(wl, device=str(dev))
+    g.imex_init(args.krylov)
+    q = g.state(wl.q)
+    heat = None if wl.heating is None else g.state(wl.heating)
+    dt = args.dt if args.dt else wl.dt
+    warm = max(1, min(args.warmup, 2))
+    g.step_ark2(q, dt, heat, warm, tol=args.tol, max_restarts=50)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start(); time.sleep(0.3)
+    ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+    stream = torch.cuda.current_stream()
+    wall0 = time.time()
+    ev0.record(stream)
+    its, rel = g.step_ark2(q, dt, heat, args.steps, tol=args.tol, max_restarts=50)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    wall1 = time.time()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), dev, world)
+    clocks = sampler.stop(wall0, wall1) if rank == 0 else None
+    finite = bool(torch.isfinite(q).all().item())
+    if rank != 0:
+        return
+    NL = wl.mesh.n_local
+    # operator applications per step: 3 S + 2 L for the stages, and per implicit stage one L per Krylov
+    # iteration plus one per restart cycle (initial residual)
+    evals = 5 * args.steps + its + 2 * args.steps
+    line = {"metric": "imex_ark2_ms_per_step", "value": ms / args.steps if finite else None, "unit": "ms/step",
+            "n_gpus": world, "steps": args.steps, "warmup": warm, "ms_per_step": ms / args.steps,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "N": wl.mesh.N, "elements": [wl.mesh.nx, wl.mesh.ny, wl.mesh.nz],
+                       "local_nodes": NL, "paper_dof": 5 * NL, "integrator": "IMEX ARK2 + GMRES(%d)" % args.krylov,
+                       "dt": dt, "gmres_tol": args.tol, "finite": finite},
+            "gmres_iterations_per_step": its / args.steps, "max_rel_residual": rel,
+            "nodal_operator_evals_gdof_per_s": 5.0 * NL * evals / (ms * 1e-3) / 1e9,
+            "clocks": clocks, "gpu_launches": int(g.launch_count),
+            "context": "PAPER.md Table 1 (L399): 0.536 s per IMEX step on 4 A100 for 165,888,000 DOF (80x80x24, N=5, "
+                       "dt=0.5 s); another machine, other inputs, an unknown GMRES tolerance: context, not a target"}
+    print(json.dumps(line))
+
+
 def kernel_alg_bytes(name, N, has_src):
     """Algorithmic bytes per local node per launch of one kernel, on SURVEY.md 8(d)'s terms (the
     stage kernels split B_alg between them; the four-call kernels count their own arrays)."""
@@ -449,6 +516,10 @@ def kernel_alg_bytes(name, N, has_src):
         return 8.0 * (5 + 5 * (2.0 / 3.0) + 5 + 5)    # q0 (2/3 of stages), qs, rhs in; q out
     if name.startswith("k_stage_volume"):
         return volume_alg_bytes(N, has_src)
+    if name.startswith("k_hd_lap"):
+        return hd_lap_alg_bytes()
+    if name.startswith("k_hd_dss"):
+        return dss_alg_bytes(N) * 4.0 / 5.0
     return 0.0
 
 
@@ -460,6 +531,12 @@ def main():
     ap.add_argument("--impl", default="numa_b200", choices=["numa_b200", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--hyperdiffusion", action="store_true", help="switch the tensor hyper-diffusion on (NEXT-1)")
+    ap.add_argument("--integrator", default="rk3", choices=["rk3", "ark2"],
+                    help="ark2: IMEX ARK2 + GMRES through numa_step_ark2 (NEXT-3); prints its own line")
+    ap.add_argument("--dt", type=float, default=0.0, help="time step for --integrator ark2 (default: the workload's)")
+    ap.add_argument("--tol", type=float, default=1e-6, help="GMRES relative residual for --integrator ark2")
+    ap.add_argument("--krylov", type=int, default=20, help="Krylov vectors per GMRES restart cycle")
     ap.add_argument("--graph", action="store_true",
                     help="launch every step as one CUDA graph (numa_step_rk3_graph; configs 1-2)")
     args = ap.parse_args()

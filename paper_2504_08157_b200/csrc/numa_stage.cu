@@ -950,7 +950,10 @@ cudaError_t stage_launch(numa_ctx *c, const StageArgs &a, cudaStream_t s)
         }
         const int64_t blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
         StageArgs a2 = a;
-        a2.pf_dist = c->n_sm * SH::MIN_BLOCKS;
+#ifndef STAGE_PF_MULT2
+#define STAGE_PF_MULT2 1   /* prefetch distance in half-waves of resident blocks (N=7: 1.605 / 1.626 / 1.732 ms at 1 / 2 / 4) */
+#endif
+        a2.pf_dist = c->n_sm * SH::MIN_BLOCKS * STAGE_PF_MULT2 / 2;
         k_stage_volume<N><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a2, c->lgl);
         return cudaGetLastError();
     }
