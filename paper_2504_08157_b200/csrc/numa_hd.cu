@@ -148,14 +148,18 @@ k_hd_lap(const double *__restrict__ f, double *out, int64_t fstride, const doubl
         for (int c = 0; c < 9; ++c) mt[c] = met[c * sm.FS + t];
 #pragma unroll
         for (int c = 0; c < 6; ++c) tt[c] = tau[c * sm.FS + t];
+        double Di[Nq], Dj[Nq], Dk[Nq];   // this node's rows of D, reused by the 4 fields
+#pragma unroll
+        for (int l = 0; l < Nq; ++l) { Di[l] = sD[i * Nq + l]; Dj[l] = sD[j * Nq + l]; Dk[l] = sD[k * Nq + l]; }
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             const double *fm = sf + m * Mn;
             double fx = 0.0, fe = 0.0, fz = 0.0;
+#pragma unroll
             for (int l = 0; l < Nq; ++l) {
-                fx = fma(sD[i * Nq + l], fm[l + Nq * (j + Nq * k)], fx);
-                fe = fma(sD[j * Nq + l], fm[i + Nq * (l + Nq * k)], fe);
-                fz = fma(sD[k * Nq + l], fm[i + Nq * (j + Nq * l)], fz);
+                fx = fma(Di[l], fm[l + Nq * (j + Nq * k)], fx);
+                fe = fma(Dj[l], fm[i + Nq * (l + Nq * k)], fe);
+                fz = fma(Dk[l], fm[i + Nq * (j + Nq * l)], fz);
             }
             const double g0 = fx * mt[0] + fe * mt[3] + fz * mt[6];
             const double g1 = fx * mt[1] + fe * mt[4] + fz * mt[7];
@@ -175,6 +179,9 @@ k_hd_lap(const double *__restrict__ f, double *out, int64_t fstride, const doubl
         for (int c = 0; c < 9; ++c) mt[c] = met[c * sm.FS + t];
         const double om = omega[t];
         double r[4];
+        double Di[Nq], Dj[Nq], Dk[Nq];
+#pragma unroll
+        for (int l = 0; l < Nq; ++l) { Di[l] = sD[i * Nq + l]; Dj[l] = sD[j * Nq + l]; Dk[l] = sD[k * Nq + l]; }
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             double div = 0.0;
@@ -182,10 +189,11 @@ k_hd_lap(const double *__restrict__ f, double *out, int64_t fstride, const doubl
             for (int c = 0; c < 3; ++c) {
                 const double *F = sF + (c * 4 + m) * Mn;
                 double fx = 0.0, fe = 0.0, fz = 0.0;
+#pragma unroll
                 for (int l = 0; l < Nq; ++l) {
-                    fx = fma(sD[i * Nq + l], F[l + Nq * (j + Nq * k)], fx);
-                    fe = fma(sD[j * Nq + l], F[i + Nq * (l + Nq * k)], fe);
-                    fz = fma(sD[k * Nq + l], F[i + Nq * (j + Nq * l)], fz);
+                    fx = fma(Di[l], F[l + Nq * (j + Nq * k)], fx);
+                    fe = fma(Dj[l], F[i + Nq * (l + Nq * k)], fe);
+                    fz = fma(Dk[l], F[i + Nq * (j + Nq * l)], fz);
                 }
                 div += fx * mt[0 + c] + fe * mt[3 + c] + fz * mt[6 + c];
             }
@@ -226,7 +234,8 @@ cudaError_t lap_launch(numa_ctx *c, const double *f, double *out, int64_t fstrid
     cudaError_t e = cudaFuncSetAttribute(k_hd_lap<Nq, SHELL, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const HdMap sm{c->shell.pos, c->shell.epb * (int)c->Mn, (int)c->shell.BS, c->shell.FS};
-    k_hd_lap<Nq, SHELL, ACC><<<(unsigned)c->par.n_elem, 256, smem, s>>>(f, out, fstride, c->met, c->hd_tau, c->omega,
+    constexpr int threads = (Nq * Nq * Nq + 31) / 32 * 32 < 256 ? (Nq * Nq * Nq + 31) / 32 * 32 : 256;
+    k_hd_lap<Nq, SHELL, ACC><<<(unsigned)c->par.n_elem, threads, smem, s>>>(f, out, fstride, c->met, c->hd_tau, c->omega,
                                                                         c->face_bc, c->lgl, sm, coef, c->has_walls);
     return cudaGetLastError();
 }

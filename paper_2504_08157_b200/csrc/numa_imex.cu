@@ -58,14 +58,18 @@ k_linop(const double *__restrict__ q, double *__restrict__ out, int64_t NL,
 #pragma unroll
         for (int c = 0; c < 9; ++c) m[c] = met[c * sm.FS + t];
         double d[5][3];
+        double Di[Nq], Dj[Nq], Dk[Nq];
+#pragma unroll
+        for (int l = 0; l < Nq; ++l) { Di[l] = sD[i * Nq + l]; Dj[l] = sD[j * Nq + l]; Dk[l] = sD[k * Nq + l]; }
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
             const double *a = sh + f * Mn;
             double fx = 0.0, fe = 0.0, fz = 0.0;
+#pragma unroll
             for (int l = 0; l < Nq; ++l) {
-                fx = fma(sD[i * Nq + l], a[l + Nq * (j + Nq * k)], fx);
-                fe = fma(sD[j * Nq + l], a[i + Nq * (l + Nq * k)], fe);
-                fz = fma(sD[k * Nq + l], a[i + Nq * (j + Nq * l)], fz);
+                fx = fma(Di[l], a[l + Nq * (j + Nq * k)], fx);
+                fe = fma(Dj[l], a[i + Nq * (l + Nq * k)], fe);
+                fz = fma(Dk[l], a[i + Nq * (j + Nq * l)], fz);
             }
             d[f][0] = fx; d[f][1] = fe; d[f][2] = fz;
         }
@@ -182,7 +186,8 @@ cudaError_t linop_launch(numa_ctx *c, const double *q, double *out, cudaStream_t
     cudaError_t e = cudaFuncSetAttribute(k_linop<Nq>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const ImMap sm{c->shell.pos, c->shell.epb * (int)c->Mn, (int)c->shell.BS, c->shell.FS};
-    k_linop<Nq><<<(unsigned)c->par.n_elem, 256, smem, s>>>(q, out, c->NL, c->ref3, c->met, c->omega, c->lgl, sm,
+    constexpr int threads = (Nq * Nq * Nq + 31) / 32 * 32 < 256 ? (Nq * Nq * Nq + 31) / 32 * 32 : 256;
+    k_linop<Nq><<<(unsigned)c->par.n_elem, threads, smem, s>>>(q, out, c->NL, c->ref3, c->met, c->omega, c->lgl, sm,
                                                           c->par.g, c->gamma);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

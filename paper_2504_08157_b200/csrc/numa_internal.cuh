@@ -59,6 +59,9 @@ struct DssLists {
     DssSeg *seg = nullptr;       // [n_seg]
     int32_t *blkmap = nullptr;   // [blocks] segment of every thread block of the DSS kernel
     int64_t n_shared = 0, n_seg = 0, blocks = 0;
+    // slab pipeline of the fused stage: DSS thread blocks [slab_blk[k], slab_blk[k+1]) hold the shared
+    // nodes whose LAST copy lies in slab k (volume blocks [slab_vol[k], slab_vol[k+1])); host side
+    std::vector<int64_t> slab_blk, slab_vol;
 };
 
 // Block-shell layout of every per-node device array the library keeps or works on
@@ -84,6 +87,7 @@ struct GraphKey { const double *q = nullptr, *heat = nullptr; void *scratch = nu
 struct numa_ctx {
     numa_params par;
     int device = 0;
+    int n_slabs = 0;   // slabs of the fused stage's volume/DSS pipeline (numa_params.reserved; 0 = one launch)
     int n_sm = 148;   // multiprocessors of `device` (grid of the persistent kernels)
     int Nq;
     int64_t Mn, NL;
@@ -160,10 +164,10 @@ cudaError_t launch_rk(numa_ctx *c, double a0, double a1, double b_dt, const doub
 // block-shell arrays [5][shell.FS]; heat is block-shell [shell.FS] or nullptr.
 cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
                                 const double *qs, const double *heat, double *qout,
-                                cudaStream_t s);
+                                cudaStream_t s, int64_t blk0 = 0, int64_t nblk = -1);
 // in-place DSS of r[5][stride] over one list set (kernel_id = profiling slot)
 cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_t stride,
-                               int kernel_id, cudaStream_t s, int nf = 5);
+                               int kernel_id, cudaStream_t s, int nf = 5, int64_t blk0 = 0, int64_t nblk = -1);
 // hyper-diffusion inside a fused stage (numa_hd.cu): h1 = DSS(omega L(qs[1..4])) before the volume
 // kernel; qout[1..4] += -b_dt P(omega L(h1)) after it (block-shell arrays)
 cudaError_t hd_stage_first(numa_ctx *c, const double *qs, cudaStream_t s);

@@ -146,6 +146,7 @@ struct StageArgs {
     double eos[14];  // binomial(gamma, n), n = 1..14: (1+x)^gamma - 1 = sum_n eos[n-1] x^n
     int has_walls;
     int pf_dist;     // blocks resident on the device: block b prefetches the phase-A inputs of block b + pf_dist
+    int64_t blk0, n_blocks;   // first block of this launch (slab pipeline) and blocks of the whole mesh
 };
 
 // Eq. 3 in cancellation-free form (Q6): p'/p0 = (1+x)^gamma - 1 with
@@ -314,8 +315,9 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 
     const int tid = threadIdx.x;
     const int64_t NL = A.GFS;                                  // field stride of every array
-    const int64_t rec = (int64_t)blockIdx.x * SH::BS;          // this block's record
-    const int64_t e0 = (int64_t)blockIdx.x * SH::EPB;
+    const int64_t bid = A.blk0 + blockIdx.x;                   // block of the mesh (a launch may cover a slab)
+    const int64_t rec = bid * SH::BS;                          // this block's record
+    const int64_t e0 = bid * SH::EPB;
     const int n_elems = (A.Ne - e0 < SH::EPB) ? (int)(A.Ne - e0) : SH::EPB;  // ragged last block
     const int n_lines = n_elems * N2;
 
@@ -335,7 +337,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
             if (A.heat) l2_prefetch(A.heat + rec, RB);
             if (A.beta) l2_prefetch(A.beta + rec, RB);
         }
-        if ((STAGE_L2PF & 2) && (int64_t)blockIdx.x + A.pf_dist < (int64_t)gridDim.x) {
+        if ((STAGE_L2PF & 2) && bid + A.pf_dist < A.n_blocks) {
             const int64_t rec2 = rec + (int64_t)A.pf_dist * SH::BS;
 #pragma unroll
             for (int c = 0; c < 5; ++c) l2_prefetch(A.qs + c * NL + rec2, RB);
@@ -877,10 +879,11 @@ template <int F>
 __global__ void __launch_bounds__(NUMA_DSS_THREADS, NUMA_DSS_MINB)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
             const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
-            const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL)
+            const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL, int blk_off)
 {
-    const DssSeg sg = segs[blkmap[blockIdx.x]];
-    const int t = (blockIdx.x - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
+    const int bid = blk_off + (int)blockIdx.x;
+    const DssSeg sg = segs[blkmap[bid]];
+    const int t = (bid - sg.blk0) * NUMA_DSS_THREADS + threadIdx.x;
     if (t >= sg.n) return;
     double *rm = r;
     if (sg.cls == 0) {
@@ -948,8 +951,10 @@ cudaError_t stage_launch(numa_ctx *c, const StageArgs &a, cudaStream_t s)
             if (e != cudaSuccess) return e;
             c->attr_stage = true;
         }
-        const int64_t blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
+        const int64_t all_blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
+        const int64_t blocks = (a.n_blocks >= 0) ? a.n_blocks : all_blocks - a.blk0;   // n_blocks carries the launch size here
         StageArgs a2 = a;
+        a2.n_blocks = all_blocks;
 #ifndef STAGE_PF_MULT2
 #define STAGE_PF_MULT2 1   /* prefetch distance in half-waves of resident blocks (N=7: 1.605 / 1.626 / 1.732 ms at 1 / 2 / 4) */
 #endif
@@ -979,7 +984,8 @@ int stage_epb(int N)
 }
 
 cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, const double *q0,
-                                const double *qs, const double *heat, double *qout, cudaStream_t s)
+                                const double *qs, const double *heat, double *qout, cudaStream_t s,
+                                int64_t blk0, int64_t nblk)
 {
     LaunchScope ls(c, K_FUSED_VOLUME, s);
     StageArgs a;
@@ -993,6 +999,7 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
     a.a0 = a0; a.a1 = a1; a.b_dt = b_dt;
     a.has_walls = c->has_walls;
     a.pf_dist = 0;
+    a.blk0 = blk0; a.n_blocks = nblk;
     // binomial(gamma, n): c_1 = gamma, c_{n+1} = c_n (gamma - n) / (n + 1)
     {
         long double cn = (long double)c->gamma;
@@ -1014,16 +1021,17 @@ cudaError_t launch_stage_volume(numa_ctx *c, double a0, double a1, double b_dt, 
 }
 
 cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_t stride,
-                               int kernel_id, cudaStream_t s, int nf)
+                               int kernel_id, cudaStream_t s, int nf, int64_t blk0, int64_t nblk)
 {
-    if (L.blocks == 0) return cudaSuccess;
+    if (nblk < 0) nblk = L.blocks - blk0;
+    if (nblk <= 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
     if (nf == 5)
-        k_stage_dss<5><<<(unsigned)L.blocks, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
-                                                                      L.copies, stride);
+        k_stage_dss<5><<<(unsigned)nblk, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
+                                                                  L.copies, stride, (int)blk0);
     else if (nf == 4)
-        k_stage_dss<4><<<(unsigned)L.blocks, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
-                                                                      L.copies, stride);
+        k_stage_dss<4><<<(unsigned)nblk, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
+                                                                  L.copies, stride, (int)blk0);
     else
         return cudaErrorInvalidValue;
     return cudaGetLastError();
