@@ -20,7 +20,11 @@
  * identity sum(wJ) = |Omega|, free stream, atmosphere at rest (bitwise zero), buoyancy
  * closed form, global mass conservation, DSS projection algebra vs an explicit Q Q^T,
  * manufactured-solution convergence order, RK3 amplification polynomial, linear
- * acoustics speed, wall projection, and a NumPy Kronecker brute-force restatement.
+ * acoustics speed, wall projection, and a NumPy Kronecker brute-force restatement (P1-P16);
+ * orc_sources: Coriolis turns the wind clockwise by f t and conserves its speed, the sponge
+ * decays as exp(-beta t) and leaves rho' alone, heating raises theta' only (P17-P19);
+ * RI diagnostic (P20-P25), hyper-diffusion (P26-P31), IMEX linear operator / ARK2 / GMRES
+ * (P32-P36) -- see the test files named at each function.
  * Physical fidelity of the tropical-cyclone run itself is "parity unpinned" (the observed
  * heating data of PAPER.md:L312 is not available).
  *

@@ -113,8 +113,7 @@ def load_library(path: str | None = None):
 
 
 def make_params(N, n_elem, n_global, constants, f_cor=0.0, method=0, eqn_set=0) -> NumaParams:
-    # NUMA_B200_SLABS: development knob for the slab pipeline of the fused stage (0 = library default)
-    return NumaParams(N=N, method=method, eqn_set=eqn_set, reserved=int(os.environ.get("NUMA_B200_SLABS", "0")), n_elem=n_elem,
+    return NumaParams(N=N, method=method, eqn_set=eqn_set, reserved=0, n_elem=n_elem,
                       n_global=n_global, g=constants["g"], p_a=constants["p_a"],
                       R_gas=constants["R_gas"], c_p=constants["c_p"], c_v=constants["c_v"],
                       f_cor=f_cor)

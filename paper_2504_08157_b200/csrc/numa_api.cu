@@ -290,10 +290,8 @@ __global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *_
 #else
         const uint64_t cls = (c == 2) ? 0 : (c == 4) ? 1 : (c == 8) ? 2 : 3;
 #endif
-        // chunk of the LAST copy: a node is complete once the volume kernel has written the slab that
-        // holds its last copy (slab pipeline of the fused stage); order inside a segment by first copy
-        const uint32_t first = (uint32_t)copies[s], last = (uint32_t)copies[s + c - 1];
-        keys[t] = ((uint64_t)(last / chunk) << 34) | (cls << 32) | first;
+        const uint32_t first = (uint32_t)copies[s];
+        keys[t] = ((uint64_t)(first / chunk) << 34) | (cls << 32) | first;
     }
 }
 
@@ -482,27 +480,6 @@ static bool build_dss_lists(numa_ctx *c, DssLists &D, const int32_t *cg, int64_t
         errstr = "internal: DSS tables do not fit";
         return false;
     }
-    // slab tables: slab k = volume blocks [k*bps, (k+1)*bps), bps a whole number of chunks, and the DSS
-    // blocks of the segments whose chunk (of the last copy) falls inside it
-    {
-        const int64_t BSp = c->shell.BS, nvb = c->shell.n_blocks;
-        int n_slabs = c->n_slabs > 0 ? c->n_slabs : 1;
-        const int64_t bpc = std::max<int64_t>(1, (int64_t)chunk / BSp);          // volume blocks per chunk
-        int64_t bps = (nvb + n_slabs - 1) / n_slabs;
-        bps = (bps + bpc - 1) / bpc * bpc;
-        D.slab_vol.clear(); D.slab_blk.clear();
-        if (n_pos == c->shell.FS && bps > 0) {
-            int k = 0;
-            for (int64_t v0 = 0; v0 < nvb; v0 += bps) {
-                D.slab_vol.push_back(v0);
-                const int64_t chunk0 = v0 * BSp / (int64_t)chunk;
-                while (k < n_seg && (int64_t)(h_hi[k] >> 2) < chunk0) ++k;
-                D.slab_blk.push_back(k < n_seg ? h_seg[k].blk0 : blk);
-            }
-            D.slab_vol.push_back(nvb);
-            D.slab_blk.push_back(blk);
-        }
-    }
     D.n_seg = n_seg;
     D.blocks = blk;
     CK(cudaMemcpyAsync(D.seg, h_seg.data(), (size_t)n_seg * sizeof(DssSeg), cudaMemcpyHostToDevice, s));
@@ -622,7 +599,6 @@ extern "C" numa_status numa_init_geometry(const numa_params *p, const double *xy
     cudaStream_t s = (cudaStream_t)stream;
     char *ws = (char *)workspace;
     c->par = *p;
-    c->n_slabs = p->reserved > 0 ? p->reserved : 0;   // tuning knob of the slab pipeline (0 = default)
     cudaGetDevice(&c->device);
     if (cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->n_sm < 1) c->n_sm = 148;
     c->Nq = p->N + 1;
@@ -742,22 +718,6 @@ static cudaError_t enqueue_step(numa_ctx *ctx, double *A, double *B, const doubl
         // qs) is written; second application added to the partial sums before the stage's DSS
         if (ctx->hd_on) e = hd_stage_first(ctx, qs, s);
         if (e != cudaSuccess) return e;
-        const DssLists &DL = ctx->dss_int;
-        const size_t n_slab = DL.slab_vol.size() > 1 ? DL.slab_vol.size() - 1 : 0;
-        if (!ctx->hd_on && n_slab > 1) {
-            // slab pipeline: the DSS of a slab runs right after the volume kernel has written it, while
-            // the partial sums are still in L2 (q_out may alias qs: a slab's DSS only touches nodes whose
-            // copies all lie in slabs already written, and later slabs read only their own records)
-            for (size_t k = 0; k < n_slab && e == cudaSuccess; ++k) {
-                e = launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, A, qs, heating, qo, s,
-                                        DL.slab_vol[k], DL.slab_vol[k + 1] - DL.slab_vol[k]);
-                if (e == cudaSuccess)
-                    e = launch_dss_classes(ctx, DL, qo, ctx->shell.FS, K_FUSED_DSS, s, 5, DL.slab_blk[k],
-                                           DL.slab_blk[k + 1] - DL.slab_blk[k]);
-            }
-            if (e != cudaSuccess) return e;
-            continue;
-        }
         e = launch_stage_volume(ctx, kRK3[st][0], kRK3[st][1], kRK3[st][2] * dt, A, qs, heating, qo, s);
         if (e != cudaSuccess) return e;
         if (ctx->hd_on) e = hd_stage_second(ctx, kRK3[st][2] * dt, qo, s);

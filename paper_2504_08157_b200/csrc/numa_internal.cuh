@@ -59,9 +59,6 @@ struct DssLists {
     DssSeg *seg = nullptr;       // [n_seg]
     int32_t *blkmap = nullptr;   // [blocks] segment of every thread block of the DSS kernel
     int64_t n_shared = 0, n_seg = 0, blocks = 0;
-    // slab pipeline of the fused stage: DSS thread blocks [slab_blk[k], slab_blk[k+1]) hold the shared
-    // nodes whose LAST copy lies in slab k (volume blocks [slab_vol[k], slab_vol[k+1])); host side
-    std::vector<int64_t> slab_blk, slab_vol;
 };
 
 // Block-shell layout of every per-node device array the library keeps or works on
@@ -87,7 +84,6 @@ struct GraphKey { const double *q = nullptr, *heat = nullptr; void *scratch = nu
 struct numa_ctx {
     numa_params par;
     int device = 0;
-    int n_slabs = 0;   // slabs of the fused stage's volume/DSS pipeline (numa_params.reserved; 0 = one launch)
     int n_sm = 148;   // multiprocessors of `device` (grid of the persistent kernels)
     int Nq;
     int64_t Mn, NL;

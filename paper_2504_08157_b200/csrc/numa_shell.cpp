@@ -72,6 +72,20 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
         }
     }
     for (int t = npb; t < nb; ++t) blocks.push_back(std::vector<int>(1, -1));
+#ifndef NUMA_SHELL_COMPACT
+#define NUMA_SHELL_COMPACT 0
+#endif
+    // COMPACT: all face / edge / corner runs at the front of the record (one contiguous region that
+    // the DSS touches), interior nodes and pads behind them; blocks then only trade places inside
+    // their zone
+    std::vector<int> zone(blocks.size(), 0);
+    if (NUMA_SHELL_COMPACT) {
+        std::vector<std::vector<int>> sh, in;
+        for (auto &b : blocks) ((b.size() > 1 || (b[0] >= 0 && ent[b[0] % Mn] != 0)) ? sh : in).push_back(b);
+        blocks = sh;
+        blocks.insert(blocks.end(), in.begin(), in.end());
+        for (size_t b = 0; b < blocks.size(); ++b) zone[b] = b < sh.size() ? 1 : 0;
+    }
     std::vector<int> seq(nb), start(blocks.size());
     auto flatten = [&]() {
         int t = 0;
@@ -125,7 +139,7 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
                 for (int tries = 0; tries < 4 && blocks[a].size() != blocks[b].size(); ++tries) b = (int)(rnd() % nblk);
                 if (blocks[a].size() != blocks[b].size()) continue;
             }
-            if (a == b) continue;
+            if (a == b || zone[a] != zone[b]) continue;
             if (a > b) std::swap(a, b);
             if (blocks[a].size() == blocks[b].size()) {
                 // equal lengths: the other blocks stay where they are, only the groups under the
