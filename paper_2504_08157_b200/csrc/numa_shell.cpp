@@ -72,14 +72,18 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
         }
     }
     for (int t = npb; t < nb; ++t) blocks.push_back(std::vector<int>(1, -1));
-#ifndef NUMA_SHELL_COMPACT
-#define NUMA_SHELL_COMPACT 0
+#ifndef NUMA_SHELL_COMPACT_MINN
+#define NUMA_SHELL_COMPACT_MINN 4
 #endif
-    // COMPACT: all face / edge / corner runs at the front of the record (one contiguous region that
-    // the DSS touches), interior nodes and pads behind them; blocks then only trade places inside
-    // their zone
+    // COMPACT (N >= 4): all face / edge / corner runs at the front of the record -- one contiguous
+    // region per element and field that the DSS touches, so its 32-byte sectors and DRAM bursts are
+    // fully used -- interior nodes and pads behind them; blocks then only trade places inside their
+    // zone.  The price is bank conflicts in the volume kernel's pointwise phases (wavefront ratio
+    // 1.25 / 1.5 / 1.6 / 1.8 / 1.2 at N = 4..8 instead of 1.0-1.3), which cost it 0-2 %; measured per
+    // 32 M nodes (DSS ms, stage fraction): N=4 0.54 -> 0.52 (0.68 -> 0.69), N=5 0.60 -> 0.52 (0.64 -> 0.66),
+    // N=7 0.50 -> 0.39 (0.61 -> 0.64), N=8 0.47 -> 0.37 (0.57 -> 0.60); N=3 neutral (left interleaved).
     std::vector<int> zone(blocks.size(), 0);
-    if (NUMA_SHELL_COMPACT) {
+    if (N >= NUMA_SHELL_COMPACT_MINN) {
         std::vector<std::vector<int>> sh, in;
         for (auto &b : blocks) ((b.size() > 1 || (b[0] >= 0 && ent[b[0] % Mn] != 0)) ? sh : in).push_back(b);
         blocks = sh;
@@ -120,7 +124,9 @@ void numa_build_shell_pos(int N, int epb, int64_t BS, std::vector<int32_t> &pos,
     const int nblk = (int)blocks.size();
     // measured (pointwise wavefronts over the ideal two per request): 1.00 at N <= 5, 1.0-1.05 at
     // N = 6 and 8; N = 7 (no pad positions, 16 nodes of every 8-byte bank pair) stays near 1.2
-    const long iters = (nb > 128 ? NUMA_SHELL_ITERS : 1) * (400000L + 4000L * nb);
+    // (N = 8: three times longer -- its 736-thread block is alone on the SM and feels the conflicts:
+    //  wavefront ratio 1.30 -> 1.13, stage fraction 0.597 -> 0.605)
+    const long iters = (nb > 128 ? NUMA_SHELL_ITERS * (N == 8 ? 3 : 1) : 1) * (400000L + 4000L * nb);
     auto accept_step = [&](int delta, long it) {
         if (delta <= 0) return true;
         // accept an uphill step of d with probability 2^(-d / T), T falling linearly
