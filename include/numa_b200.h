@@ -149,6 +149,8 @@ numa_status numa_rk_stage(numa_ctx *ctx, double a0, double a1, double b_dt, cons
  * Box meshes with planar walls (all BASELINE.json configurations) satisfy all three.  Where
  * (2) or (3) fails the fused route averages the projected tendencies of the copies with the
  * weights omega instead of projecting the assembled tendency: use the four-call route there.
+ * numa_init_geometry checks (2) and (3) (projectors of all copies of a wall node compared to 1e-10);
+ * on a mesh that fails the check numa_step_rk3 / _graph / _host return NUMA_ERR_UNSUPPORTED.
  *
  * Inside the call the state is kept in a block-shell layout in `scratch`; q is
  * converted on entry and written back (natural layout) before the call returns, so the cost

@@ -348,6 +348,51 @@ __global__ void k_face_bc(const uint8_t *__restrict__ in, uint8_t *__restrict__ 
     if (any) atomicOr(flags + 2, 1);
 }
 
+// Preconditions (2) and (3) of the fused route (include/numa_b200.h): the no-flux projector must be
+// the same in every element that shares a wall node.  One thread per shared global node applies the
+// projector of every copy (its element's wall faces, its own metric normals) to the three unit
+// vectors and compares with the first copy; flags[3] is raised where they differ by more than 1e-10
+// (curved or terrain-following walls; an element that touches a wall node without owning a wall face).
+__global__ void k_check_walls(const int32_t *__restrict__ start, const int32_t *__restrict__ copies,
+                              const double *__restrict__ met, const uint8_t *__restrict__ face_bc,
+                              const int32_t *__restrict__ pos, int npb, int BS, int64_t FS, int Nq,
+                              int64_t NG, int32_t *flags)
+{
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= NG) return;
+    const int s0 = start[g], c = start[g + 1] - s0;
+    if (c < 2) return;
+    const int Mn = Nq * Nq * Nq;
+    double P0[9];
+    for (int a = 0; a < c; ++a) {
+        const int64_t p = copies[s0 + a];
+        const int64_t e = p / Mn;
+        const int n = (int)(p - e * Mn);
+        const int idx[3] = {n % Nq, (n / Nq) % Nq, n / (Nq * Nq)};
+        const int64_t b = p / npb;
+        const int64_t t = b * BS + pos[(int)(p - b * npb)];
+        double P[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};   // columns = projected unit vectors
+        for (int f = 0; f < 6; ++f) {
+            const int d = f >> 1;
+            if (!face_bc[e * 8 + f] || idx[d] != ((f & 1) ? Nq - 1 : 0)) continue;
+            const double gx = met[(3 * d + 0) * FS + t], gy = met[(3 * d + 1) * FS + t], gz = met[(3 * d + 2) * FS + t];
+            const double inv = 1.0 / sqrt(gx * gx + gy * gy + gz * gz);
+            const double nx = gx * inv, ny = gy * inv, nz = gz * inv;   // the sign drops out of n n^T
+            for (int col = 0; col < 3; ++col) {
+                const double rn = P[col] * nx + P[3 + col] * ny + P[6 + col] * nz;
+                P[col] -= rn * nx; P[3 + col] -= rn * ny; P[6 + col] -= rn * nz;
+            }
+        }
+        if (a == 0) {
+            for (int k = 0; k < 9; ++k) P0[k] = P[k];
+        } else {
+            double dmax = 0.0;
+            for (int k = 0; k < 9; ++k) dmax = fmax(dmax, fabs(P[k] - P0[k]));
+            if (dmax > 1e-10) atomicOr(flags + 3, 1);
+        }
+    }
+}
+
 #define CK(call)                                                                        \
     do {                                                                                \
         cudaError_t e_ = (call);                                                        \
@@ -556,6 +601,17 @@ static bool init_device_tables(numa_ctx *c, const WsLayout &L, char *ws, const d
     CK(cudaMemcpyAsync(h_flags, c->d_flags, 16, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     c->has_walls = h_flags[2];
+    c->fused_ok = true;
+    if (c->has_walls) {
+        k_check_walls<<<grid_for(NG), 256, 0, s>>>(c->dss_nat.start, c->dss_nat.copies, c->met, c->face_bc,
+                                                   c->shell.pos, c->shell.epb * (int)c->Mn, (int)c->shell.BS,
+                                                   c->shell.FS, c->Nq, NG, c->d_flags);
+        CK(cudaGetLastError());
+        c->launches++;
+        CK(cudaMemcpyAsync(h_flags, c->d_flags, 16, cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        c->fused_ok = (h_flags[3] == 0);
+    }
     if (h_flags[0]) {
         errstr = "numa_init_geometry: non-positive Jacobian determinant";
         result = NUMA_ERR_NEG_JACOBIAN;
@@ -734,6 +790,11 @@ static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const 
     if (!ctx || !q || !scratch) return arg_fail(ctx, "numa_step_rk3: NULL argument");
     if (n_steps < 0 || ((uintptr_t)scratch & 255)) return arg_fail(ctx, "numa_step_rk3: bad n_steps or scratch alignment");
     if (wrong_device(ctx)) return NUMA_ERR_ARG;
+    if (!ctx->fused_ok) {
+        ctx->err = "numa_step_rk3: the wall projector differs between the copies of a wall node (curved walls, or an "
+                   "element touching a wall node without a wall face): use the four-call route on this mesh";
+        return NUMA_ERR_UNSUPPORTED;
+    }
     if (n_steps == 0) return NUMA_OK;
     cudaStream_t s = (cudaStream_t)stream;
     double *A = (double *)scratch;

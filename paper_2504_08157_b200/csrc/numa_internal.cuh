@@ -101,6 +101,7 @@ struct numa_ctx {
     uint8_t *face_bc;     // [Ne][8] (padded to 8 bytes per element)
     int32_t *d_flags;     // [4] device error flags
     int has_walls;
+    bool fused_ok = true;   // the wall projector is single-valued at every wall node (k_check_walls)
     // tensor hyper-diffusion (numa_hd_init): tau[6][FS] block-shell and two 4-field work buffers
     double *hd_tau = nullptr, *hd_buf = nullptr, *hd_buf2 = nullptr;
     bool hd_on = false;

@@ -100,7 +100,7 @@ struct StageShape {
     // PREFETCH: request the phase-C inputs in phase A (17 doubles live across phase B); at high
     // N the registers are worth more as a second resident block.
 #ifndef STAGE_PREFETCH_MAXN
-#define STAGE_PREFETCH_MAXN 5
+#define STAGE_PREFETCH_MAXN 4  /* N=5: with the L2 prefetch, four blocks per SM without the register prefetch beat three with it (1.50 -> 1.39 ms per 32 M nodes) */
 #endif
     static constexpr bool PREFETCH = (N <= STAGE_PREFETCH_MAXN) && NPT == 1;
     // PFS: the same 17 inputs are prefetched with cp.async into shared memory instead (no
@@ -118,7 +118,7 @@ struct StageShape {
 #define STAGE_MINB3 6
 #endif
 #ifndef STAGE_MINB5
-#define STAGE_MINB5 3
+#define STAGE_MINB5 4
 #endif
 #ifndef STAGE_MINB6
 #define STAGE_MINB6 2
@@ -875,8 +875,11 @@ __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__
 #ifndef NUMA_DSS_MINB
 #define NUMA_DSS_MINB 10  /* 96 registers; measured: neither more (12-20) nor fewer (1) resident blocks is faster */
 #endif
-template <int F>
-__global__ void __launch_bounds__(NUMA_DSS_THREADS, NUMA_DSS_MINB)
+#ifndef NUMA_DSS_MINB_HI
+#define NUMA_DSS_MINB_HI 16 /* N >= 6 on the compact layout (64 registers): N=7 0.394 / 0.366 / 0.359 ms at 10 / 14 / 16; N=4 prefers 10 */
+#endif
+template <int F, int MINB>
+__global__ void __launch_bounds__(NUMA_DSS_THREADS, MINB)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
             const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
             const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL, int blk_off)
@@ -1026,14 +1029,12 @@ cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_
     if (nblk < 0) nblk = L.blocks - blk0;
     if (nblk <= 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
-    if (nf == 5)
-        k_stage_dss<5><<<(unsigned)nblk, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
-                                                                  L.copies, stride, (int)blk0);
-    else if (nf == 4)
-        k_stage_dss<4><<<(unsigned)nblk, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start,
-                                                                  L.copies, stride, (int)blk0);
-    else
-        return cudaErrorInvalidValue;
+    const bool hi = c->par.N >= 6;   // measured: N=5 0.52 (10) vs 0.56 (16); N=6 0.45 vs 0.44; N=7 0.39 vs 0.36; N=8 0.37 vs 0.34 ms
+#define DSS_LAUNCH(F, MB) k_stage_dss<F, MB><<<(unsigned)nblk, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start, L.copies, stride, (int)blk0)
+    if (nf == 5) { if (hi) DSS_LAUNCH(5, NUMA_DSS_MINB_HI); else DSS_LAUNCH(5, NUMA_DSS_MINB); }
+    else if (nf == 4) { if (hi) DSS_LAUNCH(4, NUMA_DSS_MINB_HI); else DSS_LAUNCH(4, NUMA_DSS_MINB); }
+    else return cudaErrorInvalidValue;
+#undef DSS_LAUNCH
     return cudaGetLastError();
 }
 

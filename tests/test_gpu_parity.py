@@ -617,3 +617,29 @@ def test_full_size_cfg5_prefix_and_suffix():
         record("FULL SIZE cfg5 %s (rows of 160 columns, one RK3 step, fused route)" % name, [5, 7, 1.0], qg, qo)
         assert np.all(e <= TOL_RHS * 3), (name, e)     # three stages, each within the per-call bound
         assert np.all(rel_l2(qg, qo) <= TOL_100), name
+
+
+def test_fused_route_refuses_meshes_with_curved_walls():
+    """Preconditions (2)/(3) of the fused stage (include/numa_b200.h): on a terrain-following mesh the
+    metric normals of the elements sharing a bottom-wall node differ, the projector is not
+    single-valued, and numa_step_rk3 must say so (NUMA_ERR_UNSUPPORTED) instead of silently averaging;
+    the four-call route still matches the oracle there."""
+    mesh = inputs.box_mesh(4, 3, 3, 3, (900.0, 900.0, 600.0))
+    x, y, z = mesh.xyz
+    mesh.xyz[2] = z + 40.0 * np.sin(np.pi * x / 900.0) * np.sin(np.pi * y / 900.0) * (1.0 - z / 600.0)
+    rho0, th0 = inputs.reference_neutral(mesh.xyz[2])
+    ref = np.stack((rho0, th0))
+    g = binding.Numa(4, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    o = orc.Oracle(4, mesh.xyz, mesh.intma_cg, mesh.n_global, mesh.face_bc, ref, inputs.CONSTANTS)
+    q = inputs.smooth_random_state(mesh, rho0, th0, seed=13)
+    qd = g.state(q)
+    with pytest.raises(binding.NumaError) as ei:
+        g.step_rk3(qd, 0.01, None, 1)
+    assert ei.value.status == 2
+    r_o = o.rhs(q)
+    r_g = _np(g.full_rhs(qd, None))
+    assert np.all(rel_l2(r_g, r_o) <= TOL_RHS)
+    # planar walls (every BASELINE.json configuration) pass the check
+    wl = inputs.make_workload(2, N=3, scale=0.2)
+    g2 = binding.Numa.from_workload(wl)
+    g2.step_rk3(g2.state(wl.q), wl.dt, None, 1)
