@@ -175,8 +175,10 @@ numa_status numa_step_rk3_graph(numa_ctx *ctx, double *q, void *scratch, const d
  * End-to-end variant with HOST buffers: copies q (and heating, if non-NULL) host -> device
  * into caller-provided device staging buffers, runs n_steps of numa_step_rk3, copies q back
  * and synchronises.  q_host [5][Ne][Mn] (in/out), heating_host [Ne][Mn] or NULL; pinned host
- * memory gives the best copy rate.  d_q: device [5][Ne][Mn]; d_heating: device [Ne][Mn] or
- * NULL iff heating_host is NULL.
+ * memory gives the best copy rate.  d_q: device [5][Ne][Mn]; d_heating: device [Ne][Mn] or NULL.
+ * heating_host != NULL: the field is uploaded into d_heating first (a refresh); heating_host == NULL
+ * with d_heating != NULL: the heating already resident in d_heating is used (it only changes at a
+ * refresh, BASELINE.json config 3 "refreshed every 60 s"); both NULL: no heating.
  */
 numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const double *heating_host,
                                double *d_q, double *d_heating, void *scratch, double dt,

@@ -230,6 +230,7 @@ class Numa:
             d_q = torch.empty(q_host.shape, dtype=torch.float64, device=self.device)
         if heating_host is not None and d_heating is None:
             d_heating = torch.empty(heating_host.shape, dtype=torch.float64, device=self.device)
+        # heating_host None with d_heating given: the heating resident in d_heating is reused
         self._check(self.lib.numa_step_rk3_host(self.ctx, _ptr(q_host), _ptr(heating_host),
                                                 _ptr(d_q), _ptr(d_heating), _ptr(self.scratch()),
                                                 dt, n_steps, _stream()))

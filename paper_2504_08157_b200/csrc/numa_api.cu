@@ -872,8 +872,8 @@ extern "C" numa_status numa_step_rk3_host(numa_ctx *ctx, double *q_host, const d
                                           int32_t n_steps, void *stream)
 {
     if (!ctx || !q_host || !d_q || !scratch) return arg_fail(ctx, "numa_step_rk3_host: NULL argument");
-    if ((heating_host == nullptr) != (d_heating == nullptr))
-        return arg_fail(ctx, "numa_step_rk3_host: heating_host and d_heating must both be given or both NULL");
+    if (heating_host != nullptr && d_heating == nullptr)
+        return arg_fail(ctx, "numa_step_rk3_host: heating_host needs the device staging buffer d_heating");
     if (wrong_device(ctx)) return NUMA_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     const size_t nb = (size_t)ctx->NL * 8;

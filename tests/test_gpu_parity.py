@@ -436,6 +436,12 @@ def test_host_buffer_entry_point_matches_device_path():
     hh = torch.from_numpy(wl.heating.copy()).pin_memory()
     g.step_rk3_host(qh, wl.dt, hh, 2)
     assert torch.equal(qh, qd.cpu())
+    # heating resident on the device from an earlier call (no re-upload between refreshes)
+    dq = torch.empty_like(qd); dh = torch.empty_like(hd)
+    qh2 = torch.from_numpy(wl.q.copy()).pin_memory()
+    g.step_rk3_host(qh2, wl.dt, hh, 1, dq, dh)
+    g.step_rk3_host(qh2, wl.dt, None, 1, dq, dh)
+    assert torch.equal(qh2, qd.cpu())
 
 
 def test_full_size_cfg3_in_the_bench_configuration():
