@@ -360,6 +360,28 @@ def run_gpu(args):
     h2d = 5 * NL * 8 + (NL * 8 // e2e_steps if hh is not None else 0)   # average per step
     d2h = 5 * NL * 8
 
+    # ---- optional: the RI-velocity diagnostic (numa_ri_*, Eq. 18-22) on the final state -----
+    ri = None
+    if args.ri and rank == 0:
+        lev, n_lev = inputs.node_levels(mesh)
+        r_max = 0.4 * min(mesh.extent[0], mesh.extent[1])
+        g.ri_init(mesh.xyz, lev, n_lev, r_max, 50)
+        g.ri_velocity(q)
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(10):
+            out_ri = g.ri_velocity(q)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ri_ms = e0.elapsed_time(e1) / 10
+        sc = out_ri[3].cpu().numpy()
+        # per call: u, v, w, x, y, area + index per local node (centroid) and u, v, x, y + index per point
+        ri_bytes = NL * (6 * 8 + 4) + mesh.n_global * (4 * 8 + 4)
+        ri = {"ms_per_call": ri_ms, "u_ri": float(sc[0]), "max_horizontal_speed": float(sc[1]),
+              "levels": n_lev, "strips": 50, "r_max": r_max, "alg_bytes": ri_bytes,
+              "achieved_gbs": ri_bytes / (ri_ms * 1e-3) / 1e9}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -449,6 +471,8 @@ def run_gpu(args):
         "roofline": roofline,
         "cpu_baseline": cpu,
     }
+    if ri is not None:
+        line["ri_diagnostic"] = ri
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -533,6 +557,7 @@ def main():
     ap.add_argument("--impl", default="numa_b200", choices=["numa_b200", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ri", action="store_true", help="also time the RI-velocity diagnostic (NEXT-4) on the final state")
     ap.add_argument("--hyperdiffusion", action="store_true", help="switch the tensor hyper-diffusion on (NEXT-1)")
     ap.add_argument("--integrator", default="rk3", choices=["rk3", "ark2"],
                     help="ark2: IMEX ARK2 + GMRES through numa_step_ark2 (NEXT-3); prints its own line")

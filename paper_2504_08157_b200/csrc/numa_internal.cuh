@@ -24,13 +24,13 @@ struct LglTables {
 enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_HD = 7, K_HD_DSS = 8, K_COUNT = 9 };
 
 #ifndef NUMA_DSS_CHUNK
-#define NUMA_DSS_CHUNK 2048    // positions per DSS locality chunk at N <= 4
+#define NUMA_DSS_CHUNK 4096    // positions per DSS locality chunk at N <= 4 (compact layout: 0.605 / 0.515 / 0.497 / 0.504 ms at 1 K / 2 K / 4 K / 8 K on cfg3)
 #endif
 #ifndef NUMA_DSS_CHUNK_HI
 #define NUMA_DSS_CHUNK_HI 32768 // ... at N >= 5 (numa_api.cu, dss_chunk)
 #endif
 #ifndef NUMA_DSS_THREADS
-#define NUMA_DSS_THREADS 64    // shared nodes per thread block of the DSS kernel
+#define NUMA_DSS_THREADS 32    // shared nodes per thread block of the DSS kernel (cfg3: 0.492 / 0.515 / 0.536 ms at 32 / 64 / 128)
 #endif
 
 struct DssSeg {

@@ -873,10 +873,10 @@ __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__
 
 // block = NUMA_DSS_THREADS shared nodes, F fields per thread (5: the state; 4: hyper-diffusion)
 #ifndef NUMA_DSS_MINB
-#define NUMA_DSS_MINB 10  /* 96 registers; measured: neither more (12-20) nor fewer (1) resident blocks is faster */
+#define NUMA_DSS_MINB 20  /* 32-thread blocks: 640 threads per SM, 96 registers; measured: neither more nor fewer is faster at N <= 5 */
 #endif
 #ifndef NUMA_DSS_MINB_HI
-#define NUMA_DSS_MINB_HI 16 /* N >= 6 on the compact layout (64 registers): N=7 0.394 / 0.366 / 0.359 ms at 10 / 14 / 16; N=4 prefers 10 */
+#define NUMA_DSS_MINB_HI 32 /* (1024 threads per SM) N >= 6 on the compact layout (64 registers): N=7 0.394 / 0.366 / 0.359 ms at 10 / 14 / 16; N=4 prefers 10 */
 #endif
 template <int F, int MINB>
 __global__ void __launch_bounds__(NUMA_DSS_THREADS, MINB)
