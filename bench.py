@@ -91,16 +91,19 @@ def measured_peaks():
 
 def captured_traffic(workload, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the
-    tracked ncu --set full summary profiles/traffic_r2.json (written from the capture named
-    there); None when no capture of this workload / kernel is tracked."""
-    path = os.path.join(ROOT, "profiles", "traffic_r2.json")
+    tracked ncu --set full summary profiles/traffic_r2.csv (columns: workload, kernel,
+    dram_bytes_per_launch, capture; written from the captures named in its last column, commands in
+    profiles/traffic_r2.md); None when no capture of this workload / kernel is tracked."""
+    path = os.path.join(ROOT, "profiles", "traffic_r2.csv")
     try:
         with open(path) as f:
-            d = json.load(f)
-        e = d["workloads"][workload][kernel.split(" ")[0]]
-        return float(e["dram_bytes_per_launch"]), "profiles/traffic_r2.json (%s)" % e["capture"]
+            for line in f:
+                w, k, b, cap = [x.strip() for x in line.split(",")]
+                if w == workload and k == kernel.split(" ")[0]:
+                    return float(b), "profiles/traffic_r2.csv (%s)" % cap
     except Exception:
-        return None, None
+        pass
+    return None, None
 
 
 def set_omp_threads(n):
