@@ -941,7 +941,9 @@ extern "C" const char *numa_kernel_name(int32_t kernel_id)
     static const char *names[K_COUNT] = {"k_rhs (volume)", "k_dss", "k_sources", "k_rk",
                                          "k_stage_volume (fused)", "k_stage_dss (fused)",
                                          "k_shell_layout (natural <-> block-shell)",
-                                         "k_hd_lap (hyper-diffusion)", "k_hd_dss (hyper-diffusion)"};
+                                         "k_hd_lap (hyper-diffusion)", "k_hd_dss (hyper-diffusion)",
+                                         "k_linop + k_imex_walls (IMEX linear operator)",
+                                         "k_lincomb / k_dot (IMEX vector work)"};
     return (kernel_id >= 0 && kernel_id < K_COUNT) ? names[kernel_id] : "";
 }
 

@@ -187,17 +187,20 @@ cudaError_t linop_launch(numa_ctx *c, const double *q, double *out, cudaStream_t
     if (e != cudaSuccess) return e;
     const ImMap sm{c->shell.pos, c->shell.epb * (int)c->Mn, (int)c->shell.BS, c->shell.FS};
     constexpr int threads = (Nq * Nq * Nq + 31) / 32 * 32 < 256 ? (Nq * Nq * Nq + 31) / 32 * 32 : 256;
-    k_linop<Nq><<<(unsigned)c->par.n_elem, threads, smem, s>>>(q, out, c->NL, c->ref3, c->met, c->omega, c->lgl, sm,
-                                                          c->par.g, c->gamma);
+    {
+        LaunchScope ls(c, K_LINOP, s);
+        k_linop<Nq><<<(unsigned)c->par.n_elem, threads, smem, s>>>(q, out, c->NL, c->ref3, c->met, c->omega, c->lgl, sm,
+                                                              c->par.g, c->gamma);
+    }
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     e = launch_dss_classes(c, c->dss_nat, out, c->NL, K_DSS, s);
     if (e != cudaSuccess) return e;
     if (c->has_walls) {
+        LaunchScope ls(c, K_LINOP, s);
         k_imex_walls<Nq><<<(unsigned)c->par.n_elem, 128, 0, s>>>(out, c->NL, c->met, c->face_bc, sm);
         e = cudaGetLastError();
     }
-    c->launches += 2;
     return e;
 }
 
@@ -285,15 +288,20 @@ struct Imex {
     void lincomb(double *out, double c0, const double *x0, double c1 = 0, const double *x1 = nullptr, double c2 = 0,
                  const double *x2 = nullptr, double c3 = 0, const double *x3 = nullptr)
     {
-        k_lincomb<<<1184, 256, 0, s>>>(out, n5, c0, x0, c1, x1, c2, x2, c3, x3);
-        c->launches++;
+        {
+            LaunchScope ls(c, K_VEC, s);
+            k_lincomb<<<1184, 256, 0, s>>>(out, n5, c0, x0, c1, x1, c2, x2, c3, x3);
+        }
         chk(cudaGetLastError());
     }
     double dot(const double *a, const double *b)
     {
-        k_dot_partial<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(a, b, inv_mult, NL, partial);
-        k_dot_final<<<1, DOT_THREADS, 0, s>>>(partial, DOT_BLOCKS, d_scalar);
-        c->launches += 2;
+        {
+            LaunchScope ls(c, K_VEC, s);
+            k_dot_partial<<<DOT_BLOCKS, DOT_THREADS, 0, s>>>(a, b, inv_mult, NL, partial);
+            k_dot_final<<<1, DOT_THREADS, 0, s>>>(partial, DOT_BLOCKS, d_scalar);
+            c->launches += 1;
+        }
         chk(cudaGetLastError());
         double h = 0.0;
         chk(cudaMemcpyAsync(&h, d_scalar, 8, cudaMemcpyDeviceToHost, s));

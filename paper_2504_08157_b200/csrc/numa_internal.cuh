@@ -21,7 +21,7 @@ struct LglTables {
 };
 
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
-enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_HD = 7, K_HD_DSS = 8, K_COUNT = 9 };
+enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_HD = 7, K_HD_DSS = 8, K_LINOP = 9, K_VEC = 10, K_COUNT = 11 };
 
 #ifndef NUMA_DSS_CHUNK
 #define NUMA_DSS_CHUNK 4096    // positions per DSS locality chunk at N <= 4 (compact layout: 0.605 / 0.515 / 0.497 / 0.504 ms at 1 K / 2 K / 4 K / 8 K on cfg3)

@@ -561,276 +561,6 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 }
 
 // ---------------------------------------------------------------------------------------
-// Persistent variant of the volume kernel for large elements (N >= 5).  One block per SM slot
-// walks over elements e = blockIdx.x, blockIdx.x + gridDim.x, ...; while it works on element e
-// the inputs of its NEXT element are fetched into shared memory by bulk asynchronous copies
-// (cp.async.bulk, one per field: a block record of a field is one contiguous, 256-byte-aligned
-// run of BS doubles in the block-shell layout) that complete on an mbarrier:
-//   EARLY buffer = the 8 phase-A inputs (qs[5], rho0, theta0, p0), refilled right after phase A;
-//   LATE  buffer = NLATE phase-C inputs (met[9], omega | + q0[5], heat, beta = 17), refilled after
-//                  phase C.
-// The global-load latency that the plain kernel exposes at the start of phases A and C (two
-// resident blocks per SM cannot hide it: ncu long-scoreboard 43 % of all stall cycles at N=7,
-// profiles/r2a_n7_cfg4.md) is gone; the block owns the SM's registers (no spills at N=7).
-// ---------------------------------------------------------------------------------------
-template <int N>
-struct PersistShape {
-    using SH = StageShape<N>;
-#ifndef STAGE_P_EARLY_MASK
-#define STAGE_P_EARLY_MASK 0x0E0   /* bit N: EARLY buffer used (N = 5, 6, 7) */
-#endif
-#ifndef STAGE_P_LATE16_MASK
-#define STAGE_P_LATE16_MASK 0x0E0  /* bit N: all 17 late fields; otherwise met + omega only */
-#endif
-#ifndef STAGE_P_MINB5
-#define STAGE_P_MINB5 2
-#endif
-#ifndef STAGE_P_MINB6
-#define STAGE_P_MINB6 1
-#endif
-    static constexpr bool EARLY = (STAGE_P_EARLY_MASK >> N) & 1;
-    static constexpr int NLATE = ((STAGE_P_LATE16_MASK >> N) & 1) ? 17 : 10;
-    static constexpr int BS = SH::BS;
-    static constexpr int THREADS = SH::THREADS;
-    static constexpr int MIN_BLOCKS = (N == 5) ? STAGE_P_MINB5 : (N == 6) ? STAGE_P_MINB6 : 1;
-    static constexpr size_t SMEM_WORK = sizeof(double) * 3 * SH::NF * SH::FS;
-    static constexpr size_t OFF_E = (SMEM_WORK + 127) / 128 * 128;
-    static constexpr size_t OFF_L = OFF_E + (EARLY ? sizeof(double) * 8 * BS : 0);
-    static constexpr size_t OFF_BAR = OFF_L + sizeof(double) * NLATE * BS;
-    static constexpr size_t SMEM = OFF_BAR + 16;
-    static_assert(SH::EPB == 1 && SH::NPT == 1, "persistent kernel: one element per block, one node per thread");
-};
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
-{
-    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(a), "r"(parity) : "memory");
-}
-// one contiguous run of `bytes` (multiple of 16, both addresses 16-byte aligned) global -> shared
-__device__ __forceinline__ void bulk_g2s(double *sdst, const double *gsrc, unsigned bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"((unsigned)__cvta_generic_to_shared(sdst)), "l"(gsrc), "r"(bytes),
-                   "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
-}
-
-template <int N>
-__global__ void __launch_bounds__(PersistShape<N>::THREADS, PersistShape<N>::MIN_BLOCKS)
-k_stage_volume_p(const __grid_constant__ StageArgs A, const __grid_constant__ LglTables tab)
-{
-    using SH = StageShape<N>;
-    using PS = PersistShape<N>;
-    constexpr int Nq = SH::Nq, N2 = SH::N2, SJ = SH::SJ, SK = SH::SK, NF = SH::NF, FS = SH::FS,
-                  LINES = SH::LINES, BS = SH::BS;
-    constexpr unsigned REC_BYTES = BS * sizeof(double);
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *sW = reinterpret_cast<double *>(smem_raw);
-    double *sGx = sW + NF * FS;
-    double *sGe = sGx + NF * FS;
-    double *sE = reinterpret_cast<double *>(smem_raw + PS::OFF_E);   // [8][BS]
-    double *sL = reinterpret_cast<double *>(smem_raw + PS::OFF_L);   // [NLATE][BS]
-    uint64_t *barE = reinterpret_cast<uint64_t *>(smem_raw + PS::OFF_BAR);
-    uint64_t *barL = barE + 1;
-
-    const int tid = threadIdx.x;
-    const int64_t NL = A.GFS;
-    const bool same = (A.q0 == A.qs);
-    const int n_late = (PS::NLATE == 17) ? 10 + (same ? 0 : 5) + (A.heat ? 1 : 0) + (A.beta ? 1 : 0) : 10;
-
-    // this thread's node (fixed for the whole kernel): position of the record, shared index
-    const uint32_t wtab = (tid < BS) ? __ldg(A.tab + tid) : 0xFFFFFFFFu;
-    const bool has = (wtab != 0xFFFFFFFFu);
-    const int sp = (int)(wtab & 1023u), i = (int)((wtab >> 10) & 15u), j = (int)((wtab >> 14) & 15u),
-              k = (int)((wtab >> 18) & 15u);
-    const int pos = (tid & ~31) + (int)((wtab >> 26) & 31u);
-    const bool on_face = (i == 0) | (i == Nq - 1) | (j == 0) | (j == Nq - 1) | (k == 0) | (k == Nq - 1);
-    const int fp0 = A.first_pos[0];
-
-    auto issue_early = [&](int64_t e) {
-        const int64_t rec = e * BS;
-        mbar_expect_tx(barE, 8u * REC_BYTES);
-#pragma unroll
-        for (int c = 0; c < 5; ++c) bulk_g2s(sE + c * BS, A.qs + c * NL + rec, REC_BYTES, barE);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) bulk_g2s(sE + (5 + c) * BS, A.ref3 + c * NL + rec, REC_BYTES, barE);
-    };
-    auto issue_late = [&](int64_t e) {
-        const int64_t rec = e * BS;
-        mbar_expect_tx(barL, (unsigned)n_late * REC_BYTES);
-#pragma unroll
-        for (int c = 0; c < 9; ++c) bulk_g2s(sL + c * BS, A.met + c * NL + rec, REC_BYTES, barL);
-        bulk_g2s(sL + 9 * BS, A.omega + rec, REC_BYTES, barL);
-        if constexpr (PS::NLATE == 17) {
-            if (!same) {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) bulk_g2s(sL + (10 + c) * BS, A.q0 + c * NL + rec, REC_BYTES, barL);
-            }
-            if (A.heat) bulk_g2s(sL + 15 * BS, A.heat + rec, REC_BYTES, barL);
-            if (A.beta) bulk_g2s(sL + 16 * BS, A.beta + rec, REC_BYTES, barL);
-        }
-    };
-    (void)issue_early;
-
-    if (tid == 0) {
-        mbar_init(barE, 1);
-        mbar_init(barL, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-    int64_t e = blockIdx.x;
-    if (tid == 0 && e < A.Ne) {
-        if constexpr (PS::EARLY) issue_early(e);
-        issue_late(e);
-    }
-    unsigned par = 0;
-    for (; e < A.Ne; e += gridDim.x) {
-        const int64_t rec = e * BS;
-        const int64_t p = rec + pos;
-        const int64_t e2 = e + gridDim.x;
-        // ---- phase A ---------------------------------------------------------------------------
-        double qv[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, rho0 = 1.0;
-        uint2 bcw = make_uint2(0u, 0u);
-        if (A.has_walls && on_face) bcw = __ldg(reinterpret_cast<const uint2 *>(A.face_bc + e * 8));
-        if constexpr (PS::EARLY) mbar_wait(barE, par);
-        if (has) {
-            double th0, p0, th0e;
-            if constexpr (PS::EARLY) {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) qv[c] = sE[c * BS + pos];
-                rho0 = sE[5 * BS + pos]; th0 = sE[6 * BS + pos]; p0 = sE[7 * BS + pos];
-                th0e = sE[6 * BS + fp0];
-            } else {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) qv[c] = A.qs[c * NL + p];
-                rho0 = __ldg(A.ref3 + p); th0 = __ldg(A.ref3 + NL + p); p0 = __ldg(A.ref3 + 2 * NL + p);
-                th0e = __ldg(A.ref3 + NL + rec + fp0);
-            }
-            const double xx = (qv[0] * th0 + qv[4] * rho0 + qv[0] * qv[4]) / (rho0 * th0);
-            const double rho = rho0 + qv[0];
-            sW[0 * FS + sp] = p0 * eos_ratio(xx, A.gamma, A.eos);
-            sW[1 * FS + sp] = qv[1];
-            sW[2 * FS + sp] = qv[2];
-            sW[3 * FS + sp] = qv[3];
-            sW[4 * FS + sp] = qv[4] + (th0 - th0e);
-            sW[5 * FS + sp] = rho * qv[1];
-            sW[6 * FS + sp] = rho * qv[2];
-            sW[7 * FS + sp] = rho * qv[3];
-        }
-        __syncthreads();   // work fields complete; the early buffer is free again
-        if constexpr (PS::EARLY) {
-            if (tid == 0 && e2 < A.Ne) issue_early(e2);
-        }
-        // ---- phase B: line tasks (as in k_stage_volume, one element) -------------------------------
-        for (int t = tid; t < NF * LINES; t += PS::THREADS) {
-            const int f = t & 7, l2 = t >> 3;
-            const int hi = l2 / Nq, lo = l2 - hi * Nq;
-            const int base = f * FS;
-            const int bx = base + ((Nq & 1) ? SJ * lo + SK * hi : SJ * hi + SK * lo);
-            line_derivs<Nq>(sW + bx, 1, sGx + bx, tab);
-            asm volatile("" ::: "memory");   // keep the two lines' registers apart
-            line_derivs<Nq>(sW + base + lo + SK * hi, SJ, sGe + base + lo + SK * hi, tab);
-        }
-        __syncthreads();
-        for (int t = tid; t < NF * LINES; t += PS::THREADS) {
-            const int f = t & 7, l2 = t >> 3;
-            const int hi = l2 / Nq, lo = l2 - hi * Nq;
-            double *w = sW + f * FS + lo + SJ * hi;
-            line_derivs<Nq>(w, SK, w, tab);
-        }
-        __syncthreads();
-        // ---- phase C ---------------------------------------------------------------------------
-        mbar_wait(barL, par);
-        if (has) {
-            double m[9], q0v[5], om, heat, beta;
-#pragma unroll
-            for (int c = 0; c < 9; ++c) m[c] = sL[c * BS + pos];
-            om = sL[9 * BS + pos];
-            if constexpr (PS::NLATE == 17) {
-                if (!same) {
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) q0v[c] = sL[(10 + c) * BS + pos];
-                }
-                heat = A.heat ? sL[15 * BS + pos] : 0.0;
-                beta = A.beta ? sL[16 * BS + pos] : 0.0;
-            } else {
-                if (!same) {
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) q0v[c] = A.q0[c * NL + p];
-                }
-                heat = A.heat ? __ldg(A.heat + p) : 0.0;
-                beta = A.beta ? __ldg(A.beta + p) : 0.0;
-            }
-            const double rhop = qv[0], u = qv[1], v = qv[2], w = qv[3];
-            const double irho = 1.0 / (rho0 + rhop);
-            const double Ux = u * m[0] + v * m[1] + w * m[2];
-            const double Ue = u * m[3] + v * m[4] + w * m[5];
-            const double Uz = u * m[6] + v * m[7] + w * m[8];
-            const double *gx = sGx + sp, *ge = sGe + sp, *gz = sW + sp;
-            double S[5];
-            {
-                const double fx = gx[0], fe = ge[0], fz = gz[0];
-                S[1] = -(fx * m[0] + fe * m[3] + fz * m[6]) * irho;
-                S[2] = -(fx * m[1] + fe * m[4] + fz * m[7]) * irho;
-                S[3] = -(fx * m[2] + fe * m[5] + fz * m[8]) * irho - (rhop * irho) * A.g;
-            }
-#pragma unroll
-            for (int f = 1; f <= 4; ++f)
-                S[f] = ((f == 4) ? 0.0 : S[f]) - (Ux * gx[f * FS] + Ue * ge[f * FS] + Uz * gz[f * FS]);
-            {
-                double div = gx[5 * FS] * m[0] + ge[5 * FS] * m[3] + gz[5 * FS] * m[6];
-                div += gx[6 * FS] * m[1] + ge[6 * FS] * m[4] + gz[6 * FS] * m[7];
-                div += gx[7 * FS] * m[2] + ge[7 * FS] * m[5] + gz[7 * FS] * m[8];
-                S[0] = -div;
-            }
-            S[4] += heat;
-            S[1] += A.f_cor * v;
-            S[2] -= A.f_cor * u;
-            S[1] -= beta * u; S[2] -= beta * v; S[3] -= beta * w; S[4] -= beta * qv[4];
-            double r[5];
-#pragma unroll
-            for (int c = 0; c < 5; ++c) r[c] = om * S[c];
-            if (bcw.x | bcw.y) {
-                WallIO io;
-#pragma unroll
-                for (int c = 0; c < 9; ++c) io.m[c] = m[c];
-                io.r[0] = r[1]; io.r[1] = r[2]; io.r[2] = r[3];
-                wall_project_cold<Nq>(bcw, i, j, k, &io);
-                r[1] = io.r[0]; r[2] = io.r[1]; r[3] = io.r[2];
-            }
-            double *qop = A.qout + p;
-            if (same) {
-                const double a01 = A.a0 + A.a1;
-#pragma unroll
-                for (int c = 0; c < 5; ++c) qop[c * NL] = om * (a01 * qv[c]) + A.b_dt * r[c];
-            } else {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) qop[c * NL] = om * (A.a0 * q0v[c] + A.a1 * qv[c]) + A.b_dt * r[c];
-            }
-        }
-        __syncthreads();   // late buffer and derivative buffers are free again
-        if (tid == 0 && e2 < A.Ne) issue_late(e2);
-        par ^= 1u;
-    }
-}
-
-// ---------------------------------------------------------------------------------------
 // DSS by multiplicity class (Alg. 3 gather + scatter, deterministic): one thread per shared
 // global node; the copy lists of the nodes with C copies are stored transposed
 // (idx[a*n + t]) so that the index loads coalesce and carry no dependent chain; all 5*C
@@ -926,45 +656,27 @@ __global__ void k_shell_layout(const double *__restrict__ src, double *__restric
     }
 }
 
-#ifndef STAGE_PERSIST_MASK
-#define STAGE_PERSIST_MASK 0x000   /* bit N set = the persistent bulk-copy kernel (measured slower at N = 5..8: one block per SM has too few warps) */
-#endif
-
 template <int N>
 cudaError_t stage_launch(numa_ctx *c, const StageArgs &a, cudaStream_t s)
 {
     using SH = StageShape<N>;
     if (c->shell.BS != SH::BS || c->shell.epb != SH::EPB) return cudaErrorInvalidValue;  // layout of this context
-    if constexpr (((STAGE_PERSIST_MASK >> N) & 1) && SH::EPB == 1 && SH::NPT == 1) {
-        using PS = PersistShape<N>;
-        if (!c->attr_stage) {   // per device: a context is bound to one device
-            cudaError_t e = cudaFuncSetAttribute(k_stage_volume_p<N>,
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PS::SMEM);
-            if (e != cudaSuccess) return e;
-            c->attr_stage = true;
-        }
-        int64_t blocks = (int64_t)c->n_sm * PS::MIN_BLOCKS;
-        if (blocks > c->par.n_elem) blocks = c->par.n_elem;
-        k_stage_volume_p<N><<<(unsigned)blocks, PS::THREADS, PS::SMEM, s>>>(a, c->lgl);
-        return cudaGetLastError();
-    } else {
-        if (!c->attr_stage) {
-            cudaError_t e = cudaFuncSetAttribute(k_stage_volume<N>,
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SH::SMEM);
-            if (e != cudaSuccess) return e;
-            c->attr_stage = true;
-        }
-        const int64_t all_blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
-        const int64_t blocks = (a.n_blocks >= 0) ? a.n_blocks : all_blocks - a.blk0;   // n_blocks carries the launch size here
-        StageArgs a2 = a;
-        a2.n_blocks = all_blocks;
+    if (!c->attr_stage) {   // per device: a context is bound to one device
+        cudaError_t e = cudaFuncSetAttribute(k_stage_volume<N>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SH::SMEM);
+        if (e != cudaSuccess) return e;
+        c->attr_stage = true;
+    }
+    const int64_t all_blocks = (c->par.n_elem + SH::EPB - 1) / SH::EPB;
+    const int64_t blocks = (a.n_blocks >= 0) ? a.n_blocks : all_blocks - a.blk0;   // n_blocks carries the launch size here
+    StageArgs a2 = a;
+    a2.n_blocks = all_blocks;
 #ifndef STAGE_PF_MULT2
 #define STAGE_PF_MULT2 1   /* prefetch distance in half-waves of resident blocks (N=7: 1.605 / 1.626 / 1.732 ms at 1 / 2 / 4) */
 #endif
-        a2.pf_dist = c->n_sm * SH::MIN_BLOCKS * STAGE_PF_MULT2 / 2;
-        k_stage_volume<N><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a2, c->lgl);
-        return cudaGetLastError();
-    }
+    a2.pf_dist = c->n_sm * SH::MIN_BLOCKS * STAGE_PF_MULT2 / 2;
+    k_stage_volume<N><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a2, c->lgl);
+    return cudaGetLastError();
 }
 
 template <int N>
