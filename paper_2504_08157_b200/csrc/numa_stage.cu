@@ -146,7 +146,7 @@ struct StageArgs {
     double eos[14];  // binomial(gamma, n), n = 1..14: (1+x)^gamma - 1 = sum_n eos[n-1] x^n
     int has_walls;
     int pf_dist;     // blocks resident on the device: block b prefetches the phase-A inputs of block b + pf_dist
-    int64_t blk0, n_blocks;   // first block of this launch (slab pipeline) and blocks of the whole mesh
+    int64_t blk0, n_blocks;   // first block of this launch (a launch may cover a sub-range) and blocks of the whole mesh
 };
 
 // Eq. 3 in cancellation-free form (Q6): p'/p0 = (1+x)^gamma - 1 with
@@ -315,7 +315,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 
     const int tid = threadIdx.x;
     const int64_t NL = A.GFS;                                  // field stride of every array
-    const int64_t bid = A.blk0 + blockIdx.x;                   // block of the mesh (a launch may cover a slab)
+    const int64_t bid = A.blk0 + blockIdx.x;                   // block of the mesh (a launch may cover a sub-range)
     const int64_t rec = bid * SH::BS;                          // this block's record
     const int64_t e0 = bid * SH::EPB;
     const int n_elems = (A.Ne - e0 < SH::EPB) ? (int)(A.Ne - e0) : SH::EPB;  // ragged last block
