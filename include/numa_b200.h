@@ -172,6 +172,34 @@ numa_status numa_step_rk3_graph(numa_ctx *ctx, double *q, void *scratch, const d
                                 double dt, int32_t n_steps, void *stream);
 
 /*
+ * numa_step_rk3 for callers that cannot allocate device memory.
+ *
+ * numa_step_rk3 wants `scratch` from the caller.  A caller may have none to give: code coupled
+ * into a host model whose device memory all belongs to another runtime (OpenACC data regions, a
+ * framework pool that took the whole GPU when it started, so that a plain cudaMalloc fails), or a
+ * time loop in which cudaMalloc / cudaFree are off limits because they synchronise the device.
+ * This variant keeps the step's scratch (two block-shell states and the heating field) in an
+ * array compiled into the library, NUMA_STATIC_SCRATCH_BYTES long.  It calls no cudaMalloc,
+ * cudaFree or allocating library routine; q and heating are still the caller's (device pointers,
+ * as for numa_step_rk3), and the result is bit for bit that of numa_step_rk3.
+ *
+ *   - Limit: meshes with numa_step_scratch_bytes(p) <= NUMA_STATIC_SCRATCH_BYTES (64 MiB: about
+ *     740,000 local nodes, e.g. BASELINE.json configs 1 and 2 at N = 4).  Anything larger returns
+ *     NUMA_ERR_WORKSPACE with the two sizes in numa_last_error and runs nothing.
+ *   - Cost: every GPU the library's code is loaded on holds those 64 MiB until the process exits.
+ *   - First call on a device: looks up the array's device address (cudaGetSymbolAddress, with the
+ *     context's device current) and keeps it.  Make that first call outside any stream capture.
+ *   - One array per device, shared by every context and every call: two calls whose work overlaps
+ *     on the GPU (different streams, no ordering between them) race on it.  Calls ordered on one
+ *     stream, or separated by a synchronisation, are fine.  The array keeps the last call's
+ *     contents; no part of it has to be cleared, because each call rewrites what it later reads.
+ */
+#define NUMA_STATIC_SCRATCH_BYTES (64u << 20)
+size_t numa_static_scratch_bytes(void); /* = NUMA_STATIC_SCRATCH_BYTES of the loaded library */
+numa_status numa_step_rk3_static(numa_ctx *ctx, double *q, const double *heating, double dt,
+                                 int32_t n_steps, void *stream);
+
+/*
  * End-to-end variant with HOST buffers: copies q (and heating, if non-NULL) host -> device
  * into caller-provided device staging buffers, runs n_steps of numa_step_rk3, copies q back
  * and synchronises.  q_host [5][Ne][Mn] (in/out), heating_host [Ne][Mn] or NULL; pinned host

@@ -21,7 +21,8 @@ STATUS = {0: "NUMA_OK", 1: "NUMA_ERR_ARG", 2: "NUMA_ERR_UNSUPPORTED", 3: "NUMA_E
 # product ABI (include/numa_b200.h) and measurement ABI (include/numa_b200_measure.h)
 EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometry", "numa_rhs",
            "numa_dss_or_flux", "numa_apply_sources", "numa_rk_stage", "numa_step_rk3",
-           "numa_step_rk3_graph", "numa_step_rk3_host", "numa_copy_table", "numa_destroy",
+           "numa_step_rk3_graph", "numa_step_rk3_host", "numa_step_rk3_static",
+           "numa_static_scratch_bytes", "numa_copy_table", "numa_destroy",
            "numa_last_error", "numa_ri_workspace_bytes", "numa_ri_init", "numa_ri_velocity",
            "numa_ri_destroy", "numa_hd_workspace_bytes", "numa_hd_init", "numa_hyperdiffusion",
            "numa_imex_workspace_bytes", "numa_imex_init", "numa_linear_operator", "numa_step_ark2"]
@@ -69,6 +70,9 @@ def load_library(path: str | None = None):
     L.numa_step_rk3.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_graph.argtypes = [vp, dp, vp, dp, C.c_double, C.c_int32, vp]
     L.numa_step_rk3_host.argtypes = [vp, dp, dp, dp, dp, vp, C.c_double, C.c_int32, vp]
+    L.numa_step_rk3_static.argtypes = [vp, dp, dp, C.c_double, C.c_int32, vp]
+    L.numa_static_scratch_bytes.argtypes = []
+    L.numa_static_scratch_bytes.restype = C.c_size_t
     L.numa_copy_table.argtypes = [vp, C.c_int32, dp, vp]
     L.numa_imex_workspace_bytes.argtypes = [C.POINTER(NumaParams), C.c_int32]
     L.numa_imex_workspace_bytes.restype = C.c_size_t
@@ -103,7 +107,7 @@ def load_library(path: str | None = None):
     L.numa_last_error.restype = C.c_char_p
     for f in ("numa_init_geometry", "numa_rhs", "numa_dss_or_flux", "numa_apply_sources",
               "numa_rk_stage", "numa_step_rk3", "numa_step_rk3_graph", "numa_step_rk3_host",
-              "numa_copy_table", "numa_ri_init", "numa_ri_velocity", "numa_ri_destroy",
+              "numa_step_rk3_static", "numa_copy_table", "numa_ri_init", "numa_ri_velocity", "numa_ri_destroy",
               "numa_hd_init", "numa_hyperdiffusion", "numa_imex_init", "numa_linear_operator",
               "numa_step_ark2", "numa_destroy"):
         getattr(L, f).restype = C.c_int
@@ -222,6 +226,13 @@ class Numa:
     def step_rk3(self, q, dt, heating=None, n_steps=1, graph=False):
         fn = self.lib.numa_step_rk3_graph if graph else self.lib.numa_step_rk3
         self._check(fn(self.ctx, _ptr(q), _ptr(self.scratch()), _ptr(heating), dt, n_steps, _stream()))
+        return q
+
+    def step_rk3_static(self, q, dt, heating=None, n_steps=1):
+        """numa_step_rk3_static: step_rk3 on the library's built-in scratch array, for callers that
+        cannot allocate device memory (no torch scratch tensor is created; meshes beyond
+        numa_static_scratch_bytes() raise NUMA_ERR_WORKSPACE)."""
+        self._check(self.lib.numa_step_rk3_static(self.ctx, _ptr(q), _ptr(heating), dt, n_steps, _stream()))
         return q
 
     def step_rk3_host(self, q_host, dt, heating_host=None, n_steps=1, d_q=None, d_heating=None):

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnuma_b200.so")
-SOURCES = ["numa_api.cu", "numa_kernels.cu", "numa_stage.cu", "numa_measure.cu", "numa_ri.cu", "numa_hd.cu", "numa_imex.cu", "numa_shell.cpp"]
+SOURCES = ["numa_api.cu", "numa_kernels.cu", "numa_stage.cu", "numa_measure.cu", "numa_ri.cu", "numa_hd.cu", "numa_imex.cu", "numa_static_scratch.cu", "numa_shell.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
