@@ -50,7 +50,8 @@ typedef enum {
     NUMA_ERR_UNSUPPORTED = 2,  /* method = DG / eqn_set = conservative (not built) */
     NUMA_ERR_CUDA = 3,         /* CUDA runtime or launch error, or no device                 */
     NUMA_ERR_NEG_JACOBIAN = 4, /* some node has det(dx/dxi) <= 0                             */
-    NUMA_ERR_WORKSPACE = 5     /* workspace too small or misaligned                          */
+    NUMA_ERR_WORKSPACE = 5,    /* workspace too small or misaligned                          */
+    NUMA_ERR_NOT_CONVERGED = 6 /* numa_step_ark2: GMRES above tol after the last restart     */
 } numa_status;
 
 typedef struct {
@@ -70,8 +71,9 @@ typedef struct {
 /* Bytes of device workspace numa_init_geometry needs for these parameters (0 on bad input). */
 size_t numa_workspace_bytes(const numa_params *p);
 
-/* Bytes of device scratch numa_step_rk3 needs (two state-sized buffers in the block-shell
- * layout: the state of the step and the stage state). */
+/* Bytes of device scratch numa_step_rk3 needs: two state-sized buffers in the block-shell
+ * layout (the state of the step and the stage state) PLUS one field for the heating.  Always
+ * size scratch with this call; numa_step_rk3 has no size argument to check it against. */
 size_t numa_step_scratch_bytes(const numa_params *p);
 
 /*
@@ -157,7 +159,8 @@ numa_status numa_rk_stage(numa_ctx *ctx, double a0, double a1, double b_dt, cons
  * of the two conversions is amortised over n_steps.
  * heating may be NULL; it is held constant over the n_steps (the caller refreshes it between
  * calls: BASELINE.json config 3 "refreshed every 60 s").
- * scratch: >= numa_step_scratch_bytes(p) bytes (two states), 256-byte aligned.
+ * scratch: >= numa_step_scratch_bytes(p) bytes (two states plus one field for the heating),
+ * 256-byte aligned.
  *
  * numa_step_rk3_graph: the same steps with the three stages of a step captured once into a
  * CUDA graph (cached in the context, keyed by the pointer arguments, dt and stream) and
@@ -269,8 +272,13 @@ numa_status numa_hyperdiffusion(numa_ctx *ctx, const double *q, double *rhs, voi
  * numa_linear_operator (enqueue only): Lq = L_h(q), both [5][Ne][Mn]; Lq must not alias q.
  * numa_step_ark2 (SYNCHRONISES `stream`: every GMRES inner product is read back by the host):
  *   n_steps ARK2 steps of size dt in place on q[5][Ne][Mn]; S is evaluated through the four-call
- *   route.  gmres_iterations / max_rel_residual (host pointers, may be NULL) receive the total
- *   number of Krylov iterations and the largest final relative residual of the implicit solves.
+ *   route, including the hyper-diffusion H_q when numa_hd_init switched it on (H stays in the
+ *   explicit part: dt times its spectral radius must respect the explicit stability limit).
+ *   gmres_iterations / max_rel_residual (host pointers, may be NULL) receive the total
+ *   number of Krylov iterations and the largest final relative residual of the implicit solves
+ *   (the Givens estimate of a converged solve; the recomputed ||b - A x|| / ||b|| of one that ran
+ *   out of restarts).  If any solve ends above tol the call still completes its n_steps, q holds
+ *   their result, and the return value is NUMA_ERR_NOT_CONVERGED (text in numa_last_error).
  */
 size_t numa_imex_workspace_bytes(const numa_params *p, int32_t m);
 numa_status numa_imex_init(numa_ctx *ctx, int32_t m, void *imex_workspace, size_t workspace_bytes,

@@ -16,7 +16,7 @@ from . import build as _build
 _LIB = None
 
 STATUS = {0: "NUMA_OK", 1: "NUMA_ERR_ARG", 2: "NUMA_ERR_UNSUPPORTED", 3: "NUMA_ERR_CUDA",
-          4: "NUMA_ERR_NEG_JACOBIAN", 5: "NUMA_ERR_WORKSPACE"}
+          4: "NUMA_ERR_NEG_JACOBIAN", 5: "NUMA_ERR_WORKSPACE", 6: "NUMA_ERR_NOT_CONVERGED"}
 
 # product ABI (include/numa_b200.h) and measurement ABI (include/numa_b200_measure.h)
 EXPORTS = ["numa_workspace_bytes", "numa_step_scratch_bytes", "numa_init_geometry", "numa_rhs",
@@ -48,9 +48,8 @@ def load_library(path: str | None = None):
     global _LIB
     if _LIB is not None and path is None:
         return _LIB
-    # NUMA_B200_LIB: development knob to load a differently tuned build of the library
-    libpath = path or os.environ.get("NUMA_B200_LIB") or _build.LIB
-    if path is None and not os.environ.get("NUMA_B200_LIB") and (not os.path.exists(libpath) or os.environ.get("NUMA_B200_REBUILD")):
+    libpath = path or _build.LIB
+    if path is None and not os.path.exists(libpath):
         libpath = _build.build()
     if not os.path.exists(libpath):
         raise ImportError("libnuma_b200.so is missing and could not be built; there is no "

@@ -285,11 +285,7 @@ __global__ void k_class_keys(const int32_t *__restrict__ nodes, const int32_t *_
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
         const int32_t g = nodes[t];
         const int32_t s = start[g], c = start[g + 1] - s;
-#ifdef NUMA_DSS_NOCLASS
-        const uint64_t cls = 3;
-#else
         const uint64_t cls = (c == 2) ? 0 : (c == 4) ? 1 : (c == 8) ? 2 : 3;
-#endif
         const uint32_t first = (uint32_t)copies[s];
         keys[t] = ((uint64_t)(first / chunk) << 34) | (cls << 32) | first;
     }
@@ -828,6 +824,7 @@ static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const 
             CKC(cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
             const int64_t l0 = ctx->launches;
             cudaError_t e = enqueue_step(ctx, A, B, H, dt, cs);
+            ctx->graph_launches = ctx->launches - l0;   // what one replay runs (same count as the plain route)
             ctx->launches = l0;  // capture enqueues nothing
             cudaError_t e2 = cudaStreamEndCapture(cs, &g);
             if (e != cudaSuccess || e2 != cudaSuccess) {
@@ -841,7 +838,7 @@ static numa_status step_rk3_impl(numa_ctx *ctx, double *q, void *scratch, const 
         }
         for (int step = 0; step < n_steps; ++step) {
             CKC(cudaGraphLaunch(ctx->graph, cs));
-            ctx->launches += ctx->hd_on ? 18 : 6;  // kernels replayed per step
+            ctx->launches += ctx->graph_launches;  // kernels replayed per step
         }
         if (cs != s) {
             CKC(cudaEventRecord(ctx->gev1, cs));

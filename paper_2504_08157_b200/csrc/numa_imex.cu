@@ -12,6 +12,7 @@
 //        preconditioner, initial guess = the stage's right-hand side, inner product = the
 //        Euclidean one over the unique global nodes (local copies weighted 1/multiplicity).
 // All vectors are natural-layout states [5][Ne][Mn]; the nonlinear S is the four-call route.
+#include <cstdio>
 #include <cmath>
 #include <new>
 #include <vector>
@@ -314,6 +315,9 @@ struct Imex {
     {
         chk(launch_rhs(c, q, out, s));
         chk(launch_dss_classes(c, c->dss_nat, out, NL, K_DSS, s));
+        // H_q of Eq. 1 when numa_hd_init switched it on: added to the assembled tendency before the
+        // sources and the no-flux projection, as in the four-call route; explicit part of the splitting
+        if (c->hd_on && numa_hyperdiffusion(c, q, out, s) != NUMA_OK) chk(cudaErrorUnknown);
         chk(launch_sources(c, q, heat, out, s));
     }
 };
@@ -355,13 +359,16 @@ int gmres_solve(Imex &I, double a, const double *b, double *x, double **V, doubl
                 H[(size_t)i * m + k] = t;
             }
             const double d = std::hypot(H[(size_t)k * m + k], H[(size_t)(k + 1) * m + k]);
+            // breakdown: column k of the rotated Hessenberg matrix is zero, so V[k] adds nothing to
+            // the span; the solution is taken from the first k columns (k_used stays k)
+            if (d == 0.0) break;
             cs[k] = H[(size_t)k * m + k] / d; sn[k] = H[(size_t)(k + 1) * m + k] / d;
             H[(size_t)k * m + k] = d; H[(size_t)(k + 1) * m + k] = 0.0;
             g[k + 1] = -sn[k] * g[k]; g[k] = cs[k] * g[k];
             ++its;
             k_used = k + 1;
             rel = std::fabs(g[k + 1]) / bnorm;
-            if (rel <= tol || d == 0.0) break;
+            if (rel <= tol) break;
             if (k + 1 < m) I.lincomb(V[k + 1], 1.0 / hn, w);
         }
         for (int i = k_used - 1; i >= 0; --i) {
@@ -371,6 +378,12 @@ int gmres_solve(Imex &I, double a, const double *b, double *x, double **V, doubl
         }
         for (int i = 0; i < k_used; ++i) I.lincomb(x, 1.0, x, y[i], V[i]);
         if (rel <= tol) break;
+    }
+    if (rel > tol && I.err == cudaSuccess) {
+        // restarts exhausted: report the true residual ||b - A x|| / ||b||, not the Givens estimate
+        apply(x, r);
+        I.lincomb(r, 1.0, b, -1.0, r);
+        rel = std::sqrt(I.dot(r, r)) / bnorm;
     }
     *rel_out = rel;
     return its;
@@ -432,5 +445,12 @@ extern "C" numa_status numa_step_ark2(numa_ctx *ctx, double *q, const double *he
     if (max_rel_residual) *max_rel_residual = rel_max;
     if (I.err == cudaSuccess) I.chk(cudaStreamSynchronize(I.s));
     if (I.err != cudaSuccess) { ctx->err = cudaGetErrorString(I.err); cudaGetLastError(); return NUMA_ERR_CUDA; }
+    if (!(rel_max <= tol)) {
+        char buf[200];
+        snprintf(buf, sizeof buf, "numa_step_ark2: GMRES left a relative residual of %.3e > tol = %.3e after %d restart(s) "
+                 "of %d vectors; q holds the steps taken with those solves", rel_max, tol, (int)max_restarts, m);
+        ctx->err = buf;
+        return NUMA_ERR_NOT_CONVERGED;
+    }
     return NUMA_OK;
 }

@@ -23,15 +23,9 @@ struct LglTables {
 // kernel ids of the optional per-kernel CUDA-event timing (numa_profile_*)
 enum { K_VOLUME = 0, K_DSS = 1, K_SOURCES = 2, K_RK = 3, K_FUSED_VOLUME = 4, K_FUSED_DSS = 5, K_LAYOUT = 6, K_HD = 7, K_HD_DSS = 8, K_LINOP = 9, K_VEC = 10, K_COUNT = 11 };
 
-#ifndef NUMA_DSS_CHUNK
 #define NUMA_DSS_CHUNK 4096    // positions per DSS locality chunk at N <= 4 (compact layout: 0.605 / 0.515 / 0.497 / 0.504 ms at 1 K / 2 K / 4 K / 8 K on cfg3)
-#endif
-#ifndef NUMA_DSS_CHUNK_HI
 #define NUMA_DSS_CHUNK_HI 32768 // ... at N >= 5 (numa_api.cu, dss_chunk)
-#endif
-#ifndef NUMA_DSS_THREADS
 #define NUMA_DSS_THREADS 32    // shared nodes per thread block of the DSS kernel (cfg3: 0.492 / 0.515 / 0.536 ms at 32 / 64 / 128)
-#endif
 
 struct DssSeg {
     int64_t node_off;  // first node of the segment in sh_nodes
@@ -113,6 +107,7 @@ struct numa_ctx {
     std::string err;
     // CUDA graph of one SSP-RK3 step (numa_step_rk3_graph)
     cudaGraphExec_t graph = nullptr;
+    int64_t graph_launches = 0;   // kernels in the captured step (counted by enqueue_step at capture)
     GraphKey graph_key;
     cudaStream_t gstream = nullptr;   // used when the caller's stream is the legacy default stream
     cudaEvent_t gev0 = nullptr, gev1 = nullptr;

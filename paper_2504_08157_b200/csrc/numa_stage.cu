@@ -36,18 +36,10 @@ namespace {
 template <int N>
 struct StageShape {
     static constexpr int Nq = N + 1, N2 = Nq * Nq, Mn = N2 * Nq;
-#ifndef STAGE_EPB4
 #define STAGE_EPB4 1
-#endif
-#ifndef STAGE_MINB4
 #define STAGE_MINB4 6
-#endif
-#ifndef STAGE_EPB3
 #define STAGE_EPB3 2
-#endif
-#ifndef STAGE_EPB5
 #define STAGE_EPB5 1
-#endif
     static constexpr int EPB = (N == 2) ? 9 : (N == 3) ? STAGE_EPB3 : (N == 4) ? STAGE_EPB4 : (N == 5) ? STAGE_EPB5 : 1;
     // shared node index i + SJ*j + SK*k; for even Nq the k-planes are padded by one double
     static constexpr int SJ = Nq;
@@ -61,23 +53,13 @@ struct StageShape {
     // NPT nodes per thread in the pointwise phases: at high N a block of Mn threads would be
     // alone on its SM (registers, shared memory); half as many threads let two blocks overlap
     // their memory and compute phases.
-#ifndef STAGE_NPT_HI
 #define STAGE_NPT_HI 2
-#endif
-#ifndef STAGE_NPT_MINN
 #define STAGE_NPT_MINN 9  /* measured: no gain at N <= 8; kept for larger elements */
-#endif
     // THR_OVR: explicit block size where the default (one thread per node) balances the line
     // tasks badly: 8*LINES tasks per direction should fill whole rounds of THREADS threads.
-#ifndef STAGE_THREADS5
 #define STAGE_THREADS5 0
-#endif
-#ifndef STAGE_THREADS6
 #define STAGE_THREADS6 416  /* 392 line tasks per pass in one round (352 threads: 352 + 40) */
-#endif
-#ifndef STAGE_THREADS8
 #define STAGE_THREADS8 0
-#endif
     static constexpr int THR_OVR = (N == 5) ? STAGE_THREADS5 : (N == 6) ? STAGE_THREADS6 : (N == 8) ? STAGE_THREADS8 : 0;
     static constexpr int NPT = THR_OVR ? (NODES + THR_OVR - 1) / THR_OVR
                                        : (N >= STAGE_NPT_MINN) ? STAGE_NPT_HI : 1;
@@ -92,43 +74,21 @@ struct StageShape {
     // POOLED: the zeta-derivatives get their own buffer, so the line tasks of all three
     // directions form one pool without a barrier in between (better balance at low N);
     // otherwise they overwrite the work fields in place after a barrier (less shared memory).
-#ifndef STAGE_POOLED_MASK
 #define STAGE_POOLED_MASK 0x04  /* bit N set = pooled */
-#endif
     static constexpr bool POOLED = (STAGE_POOLED_MASK >> N) & 1;
     static constexpr size_t SMEM_WORK = sizeof(double) * (POOLED ? 4 : 3) * NF * FS;
     // PREFETCH: request the phase-C inputs in phase A (17 doubles live across phase B); at high
     // N the registers are worth more as a second resident block.
-#ifndef STAGE_PREFETCH_MAXN
 #define STAGE_PREFETCH_MAXN 4  /* N=5: with the L2 prefetch, four blocks per SM without the register prefetch beat three with it (1.50 -> 1.39 ms per 32 M nodes) */
-#endif
     static constexpr bool PREFETCH = (N <= STAGE_PREFETCH_MAXN) && NPT == 1;
-    // PFS: the same 17 inputs are prefetched with cp.async into shared memory instead (no
-    // registers held across phase B); used where one block per SM leaves the room (N = 6, 7).
-#ifndef STAGE_PFS_MASK
-#define STAGE_PFS_MASK 0x000  /* bit N set = use it (with the L2 prefetch it no longer pays: N = 8 1.92 -> 1.79 ms without) */
-#endif
-    static constexpr bool PFS = !PREFETCH && ((STAGE_PFS_MASK >> N) & 1);
-    // PFS_ALL: all 17 inputs (met[9], omega, q0[5], heat, beta); otherwise only met and omega
-    // (N = 8: the other 7 do not fit beside the work buffers)
-    static constexpr bool PFS_ALL = (N != 8);
-    static constexpr int NPF = PFS_ALL ? 17 : 10;
-    static constexpr size_t SMEM = SMEM_WORK + (PFS ? sizeof(double) * NPF * SLOTS : 0);
-#ifndef STAGE_MINB3
+    // (a cp.async staging of the same 17 inputs into shared memory was measured too: with the L2
+    // prefetch it no longer pays, N = 8 1.92 -> 1.79 ms without; removed, in the history)
+    static constexpr size_t SMEM = SMEM_WORK;
 #define STAGE_MINB3 6
-#endif
-#ifndef STAGE_MINB5
 #define STAGE_MINB5 4
-#endif
-#ifndef STAGE_MINB6
 #define STAGE_MINB6 2
-#endif
-#ifndef STAGE_MINB7
 #define STAGE_MINB7 2
-#endif
-#ifndef STAGE_MINB8
 #define STAGE_MINB8 1
-#endif
     static constexpr int MIN_BLOCKS = (N == 4) ? STAGE_MINB4 : (N == 3) ? STAGE_MINB3 : (N == 5) ? STAGE_MINB5
                                     : (N == 6) ? STAGE_MINB6 : (N == 7) ? STAGE_MINB7 : (N == 8) ? STAGE_MINB8 : 3;
 };
@@ -175,9 +135,7 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
     double x[Nq];
 #pragma unroll
     for (int l = 0; l < Nq; ++l) x[l] = src[sstride * l];
-#ifndef STAGE_ANTISYM_MINNQ
 #define STAGE_ANTISYM_MINNQ 7  /* N >= 6; below that the full table fits and is faster */
-#endif
     if constexpr (Nq < STAGE_ANTISYM_MINNQ) {
 #pragma unroll
         for (int m = 0; m < Nq; ++m) {
@@ -186,10 +144,7 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
             for (int l = 0; l < Nq; ++l) acc = fma(tab.D[m * Nq + l], x[l], acc);
             dst[sstride * m] = acc;
         }
-#ifndef STAGE_EVEN_ODD
 #define STAGE_EVEN_ODD 7  /* Nq from which the even-odd form is used (measured: pays at N >= 6) */
-#endif
-#if STAGE_EVEN_ODD > 0
     } else if constexpr (Nq >= STAGE_EVEN_ODD) {
         // even-odd form: half the multiplications (A, B of LglTables)
         constexpr int H = Nq / 2;
@@ -210,7 +165,6 @@ __device__ __forceinline__ void line_derivs(const double *src, int sstride, doub
             for (int l = 0; l < H; ++l) a = fma(tab.M[l], o[l], a);
             dst[sstride * H] = a;
         }
-#endif
     } else {
 #pragma unroll
         for (int m = 0; m < Nq / 2; ++m) {
@@ -250,12 +204,6 @@ __device__ __noinline__ void wall_project_cold(uint2 bcw, int i, int j, int k, W
     wall_project<Nq>(bc, i, j, k, io->m, io->r[0], io->r[1], io->r[2]);
 }
 
-__device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc)
-{
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
-}
-
 // L2 prefetch of one contiguous run (bytes a multiple of 16, address 16-byte aligned): no
 // registers, no shared memory; the later ld.global then pays the L2 latency instead of HBM's
 __device__ __forceinline__ void l2_prefetch(const double *g, unsigned bytes)
@@ -285,20 +233,9 @@ __device__ __forceinline__ NodeIx node_ix(const uint32_t *__restrict__ tab, int 
 }
 
 // Global accesses of the volume kernel: every value is used once per block, so nothing is
-// gained by allocating it in L1 (STAGE_LDMODE 0 = ld.global.nc / default stores, 1 = .cg, 2 = .cs)
-#ifndef STAGE_LDMODE
-#define STAGE_LDMODE 1
-#endif
-#if STAGE_LDMODE == 1
+// gained by allocating it in L1: ld/st .cg (measured against ld.global.nc + default stores and against .cs)
 #define VLD(p) __ldcg(p)
 #define VST(p, v) __stcg(p, v)
-#elif STAGE_LDMODE == 2
-#define VLD(p) __ldcs(p)
-#define VST(p, v) __stcs(p, v)
-#else
-#define VLD(p) __ldg(p)
-#define VST(p, v) (*(p) = (v))
-#endif
 
 template <int N>
 __global__ void __launch_bounds__(StageShape<N>::THREADS, StageShape<N>::MIN_BLOCKS)
@@ -311,7 +248,6 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     double *sW = smem;            // [NF][EPB][ME] nodal work fields, later d/dzeta
     double *sGx = sW + NF * FS;   // d/dxi
     double *sGe = sGx + NF * FS;  // d/deta
-    double *sPF = smem + SH::SMEM_WORK / sizeof(double);  // [NPF][SLOTS] cp.async prefetch (PFS)
 
     const int tid = threadIdx.x;
     const int64_t NL = A.GFS;                                  // field stride of every array
@@ -321,9 +257,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     const int n_elems = (A.Ne - e0 < SH::EPB) ? (int)(A.Ne - e0) : SH::EPB;  // ragged last block
     const int n_lines = n_elems * N2;
 
-#ifndef STAGE_L2PF
 #define STAGE_L2PF 3   /* bit 0: phase-C inputs of this block; bit 1: phase-A inputs of block b + pf_dist */
-#endif
     if (STAGE_L2PF && tid == 0) {
         constexpr unsigned RB = SH::BS * sizeof(double);
         if (STAGE_L2PF & 1) {
@@ -363,22 +297,6 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 #pragma unroll
         for (int c = 0; c < 5; ++c) qv[rr][c] = 0.0;
         if (!x.has) continue;
-        if constexpr (SH::PFS) {
-            // phase-C inputs of this node -> shared memory, asynchronously; only this thread
-            // reads them back, so cp.async.wait_group is all the synchronisation needed
-            double *d = sPF + (tid + rr * SH::THREADS);
-#pragma unroll
-            for (int c = 0; c < 9; ++c) cp_async8(d + c * SH::SLOTS, A.met + c * NL + p);
-            cp_async8(d + 9 * SH::SLOTS, A.omega + p);
-            if constexpr (SH::PFS_ALL) {
-                if (!same) {
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) cp_async8(d + (10 + c) * SH::SLOTS, A.q0 + c * NL + p);
-                }
-                if (A.heat) cp_async8(d + 15 * SH::SLOTS, A.heat + p);
-                if (A.beta) cp_async8(d + 16 * SH::SLOTS, A.beta + p);
-            }
-        }
 #pragma unroll
         for (int c = 0; c < 5; ++c) qv[rr][c] = VLD(A.qs + c * NL + p);
         if constexpr (SH::PREFETCH) {
@@ -406,7 +324,6 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
         sW[6 * FS + sp] = rho * qv[rr][2];
         sW[7 * FS + sp] = rho * qv[rr][3];
     }
-    if constexpr (SH::PFS) asm volatile("cp.async.commit_group;" ::: "memory");
     __syncthreads();
 
     // ---- phase B: line tasks (Alg. 2) ----------------------------------------------------------
@@ -441,9 +358,6 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
             const int base = f * FS + el * ME;
             const int bx = base + ((Nq & 1) ? SJ * lo + SK * hi : SJ * hi + SK * lo);
             line_derivs<Nq>(sW + bx, 1, sGx + bx, tab);
-#ifdef STAGE_SPLIT_XY
-            if constexpr (N >= STAGE_SPLIT_XY) asm volatile("" ::: "memory");  // keep the two lines' registers apart
-#endif
             line_derivs<Nq>(sW + base + lo + SK * hi, SJ, sGe + base + lo + SK * hi, tab);
         }
         __syncthreads();
@@ -465,28 +379,7 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
     if (!x.has) continue;
     const int64_t p = x.p;
     const int sp = x.sp, i = x.i, j = x.j, k = x.k;
-    if constexpr (SH::PFS) {
-        if (rr == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
-        const double *d = sPF + (tid + rr * SH::THREADS);
-#pragma unroll
-        for (int c = 0; c < 9; ++c) m[c] = d[c * SH::SLOTS];
-        om = d[9 * SH::SLOTS];
-        if constexpr (SH::PFS_ALL) {
-            if (!same) {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) q0v[c] = d[(10 + c) * SH::SLOTS];
-            }
-            heat = A.heat ? d[15 * SH::SLOTS] : 0.0;
-            beta = A.beta ? d[16 * SH::SLOTS] : 0.0;
-        } else {
-            if (!same) {
-#pragma unroll
-                for (int c = 0; c < 5; ++c) q0v[c] = VLD(A.q0 + c * NL + p);
-            }
-            heat = A.heat ? VLD(A.heat + p) : 0.0;
-            beta = A.beta ? VLD(A.beta + p) : 0.0;
-        }
-    } else if constexpr (!SH::PREFETCH) {
+    if constexpr (!SH::PREFETCH) {
 #pragma unroll
         for (int c = 0; c < 9; ++c) m[c] = VLD(A.met + c * NL + p);
         om = VLD(A.omega + p);
@@ -568,16 +461,8 @@ k_stage_volume(const __grid_constant__ StageArgs A, const __grid_constant__ LglT
 // ---------------------------------------------------------------------------------------
 
 // the copies are touched once per launch by this SM: keep them out of L1 (ld/st .cg)
-#if !defined(NUMA_DSS_CA) && !defined(NUMA_DSS_CS)
 #define DSS_LD(p) __ldcg(p)
 #define DSS_ST(p, v) __stcg(p, v)
-#elif defined(NUMA_DSS_CS)
-#define DSS_LD(p) __ldcs(p)
-#define DSS_ST(p, v) __stcs(p, v)
-#else
-#define DSS_LD(p) (*(p))
-#define DSS_ST(p, v) (*(p) = (v))
-#endif
 
 template <int C, int F>
 __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__ idx, int64_t n,
@@ -602,12 +487,8 @@ __device__ __forceinline__ void dss_node(double *rm, const int32_t *__restrict__
 }
 
 // block = NUMA_DSS_THREADS shared nodes, F fields per thread (5: the state; 4: hyper-diffusion)
-#ifndef NUMA_DSS_MINB
 #define NUMA_DSS_MINB 20  /* 32-thread blocks: 640 threads per SM, 96 registers; measured: neither more nor fewer is faster at N <= 5 */
-#endif
-#ifndef NUMA_DSS_MINB_HI
 #define NUMA_DSS_MINB_HI 32 /* (1024 threads per SM) N >= 6 on the compact layout (64 registers): N=7 0.394 / 0.366 / 0.359 ms at 10 / 14 / 16; N=4 prefers 10 */
-#endif
 template <int F, int MINB>
 __global__ void __launch_bounds__(NUMA_DSS_THREADS, MINB)
 k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
@@ -671,9 +552,7 @@ cudaError_t stage_launch(numa_ctx *c, const StageArgs &a, cudaStream_t s)
     const int64_t blocks = (a.n_blocks >= 0) ? a.n_blocks : all_blocks - a.blk0;   // n_blocks carries the launch size here
     StageArgs a2 = a;
     a2.n_blocks = all_blocks;
-#ifndef STAGE_PF_MULT2
 #define STAGE_PF_MULT2 1   /* prefetch distance in half-waves of resident blocks (N=7: 1.605 / 1.626 / 1.732 ms at 1 / 2 / 4) */
-#endif
     a2.pf_dist = c->n_sm * SH::MIN_BLOCKS * STAGE_PF_MULT2 / 2;
     k_stage_volume<N><<<(unsigned)blocks, SH::THREADS, SH::SMEM, s>>>(a2, c->lgl);
     return cudaGetLastError();

@@ -73,12 +73,16 @@ def test_rk3_steps_with_hyperdiffusion_fused_route(cfg, N, scale, c3, steps):
         qo = o.step_rk3(qo, wl.dt, wl.heating)
     heat = None if wl.heating is None else g.state(wl.heating)
     qd = g.state(wl.q)
+    n0 = g.launch_count
     g.step_rk3(qd, wl.dt, heat, steps)
+    n_plain = g.launch_count - n0
     qg = qd.cpu().numpy()
     assert np.isfinite(qg).all() and np.isfinite(qo).all()
     qd2 = g.state(wl.q)
+    n0 = g.launch_count
     g.step_rk3(qd2, wl.dt, heat, steps, graph=True)
     assert torch.equal(qd, qd2)                              # graph route: same kernels, same bits
+    assert g.launch_count - n0 == n_plain                    # ... and the same number of them counted
     for m in range(5):
         den = np.linalg.norm(qo[m])
         err = np.linalg.norm(qg[m] - qo[m]) / (den if den > 0 else 1.0)
