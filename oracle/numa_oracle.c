@@ -24,7 +24,8 @@
  * orc_sources: Coriolis turns the wind clockwise by f t and conserves its speed, the sponge
  * decays as exp(-beta t) and leaves rho' alone, heating raises theta' only (P17-P19);
  * RI diagnostic (P20-P25), hyper-diffusion (P26-P31), IMEX linear operator / ARK2 / GMRES
- * (P32-P36) -- see the test files named at each function.
+ * (P32-P36), the u . grad theta0 term of Eq. 1c and the L_theta row of the linear operator in
+ * closed form on the constant-N_BV sounding (P37) -- see the test files named at each function.
  * Physical fidelity of the tropical-cyclone run itself is "parity unpinned" (the observed
  * heating data of PAPER.md:L312 is not available).
  *
