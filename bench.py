@@ -263,6 +263,11 @@ def run_gpu(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        # replicas only: the N ranks come from torchrun, bench.py spawns nothing itself
+        raise SystemExit("bench.py --gpus %d needs %d ranks but WORLD_SIZE is %d: launch it as\n  python -m "
+                         "torch.distributed.run --nnodes=1 --nproc-per-node %d --master-addr 127.0.0.1 "
+                         "--master-port 29500 bench.py --gpus %d ..." % (args.gpus, args.gpus, world, args.gpus, args.gpus))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference "
                          "for the CPU oracle arm")
