@@ -518,101 +518,6 @@ k_stage_dss(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict
     }
 }
 
-// Software-pipelined persistent form of the same work (the one-shot kernel walks
-// blkmap -> seg -> idx -> data -> store and exits, so only one latency in four moves data).  A
-// thread block of 32 threads takes the 32-node blocks b, b + G, b + 2G, ... of the same list and
-// keeps three of them in flight: while the 5*C values of block i are being loaded it requests the
-// copy indices of block i+1 (whose segment record arrived an iteration ago) and the segment record
-// of block i+2.  Same sums in the same order as k_stage_dss: bit-identical results.
-#ifndef NUMA_DSS_PIPE_MINB
-#define NUMA_DSS_PIPE_MINB 20
-#endif
-#ifndef NUMA_DSS_PIPE_MINB_HI
-#define NUMA_DSS_PIPE_MINB_HI 20
-#endif
-#ifndef NUMA_DSS_PIPE_GRID
-#define NUMA_DSS_PIPE_GRID 20   /* resident 32-thread blocks per SM of the persistent grid */
-#endif
-struct DssNext { int64_t ib; int32_t n, cls; };   // idx_base + t, nodes of the segment, class (-1: no node)
-
-template <int C, int F>
-__device__ __forceinline__ void dss_sum_store(double *rm, const int32_t (&id)[8], int64_t NL)
-{
-    double v[F][C];
-#pragma unroll
-    for (int m = 0; m < F; ++m)
-#pragma unroll
-        for (int a = 0; a < C; ++a) v[m][a] = DSS_LD(rm + m * NL + id[a]);
-#pragma unroll
-    for (int m = 0; m < F; ++m) {
-        double s = v[m][0];
-#pragma unroll
-        for (int a = 1; a < C; ++a) s += v[m][a];
-#pragma unroll
-        for (int a = 0; a < C; ++a) DSS_ST(rm + m * NL + id[a], s);
-    }
-}
-
-template <int F, int MINB>
-__global__ void __launch_bounds__(NUMA_DSS_THREADS, MINB)
-k_stage_dss_pipe(double *r, const int32_t *__restrict__ idx, const DssSeg *__restrict__ segs,
-                 const int32_t *__restrict__ blkmap, const int32_t *__restrict__ nodes,
-                 const int32_t *__restrict__ start, const int32_t *__restrict__ copies, int64_t NL,
-                 int blk_off, int n_blk)
-{
-    const int G = (int)gridDim.x;
-    int b = (int)blockIdx.x;                       // block of the list, relative to blk_off
-    auto describe = [&](int bb, const DssSeg &sg) {
-        const int t = (blk_off + bb - sg.blk0) * NUMA_DSS_THREADS + (int)threadIdx.x;
-        DssNext d;
-        d.n = sg.n;
-        d.cls = (t < sg.n) ? sg.cls : -1;
-        // class 3 (any other multiplicity) goes through the CSR lists: ib = position in sh_nodes
-        d.ib = (sg.cls == 3) ? sg.node_off + t : sg.idx_base + t;
-        return d;
-    };
-    auto load_ids = [&](const DssNext &d, int32_t (&id)[8]) {
-        const int c = (d.cls >= 0 && d.cls < 3) ? (2 << d.cls) : 0;
-#pragma unroll
-        for (int a = 0; a < 8; ++a)
-            if (a < c) id[a] = __ldg(idx + d.ib + (int64_t)a * d.n);
-    };
-    // prologue: block i = b fully described with its indices, block i+1 described
-    DssNext cur = describe(b, segs[blkmap[blk_off + b]]);
-    int32_t id[8];
-    load_ids(cur, id);
-    DssNext nxt; nxt.cls = -1; nxt.n = 0; nxt.ib = 0;
-    if (b + G < n_blk) nxt = describe(b + G, segs[blkmap[blk_off + b + G]]);
-    for (;;) {
-        // (1) indices of block i+1, (2) values of block i, (3) segment record of block i+2
-        int32_t idn[8];
-        load_ids(nxt, idn);
-        const int b2 = b + 2 * G;
-        DssSeg sg2;
-        const bool has2 = b2 < n_blk;
-        if (cur.cls == 0) dss_sum_store<2, F>(r, id, NL);
-        else if (cur.cls == 1) dss_sum_store<4, F>(r, id, NL);
-        else if (cur.cls == 2) dss_sum_store<8, F>(r, id, NL);
-        else if (cur.cls == 3) {
-            const int gI = nodes[cur.ib];
-            const int s = start[gI], c = start[gI + 1] - s;
-            for (int m = 0; m < F; ++m) {
-                double *rf = r + (int64_t)m * NL;
-                double sum = rf[copies[s]];
-                for (int a = 1; a < c; ++a) sum += rf[copies[s + a]];
-                for (int a = 0; a < c; ++a) rf[copies[s + a]] = sum;
-            }
-        }
-        if (has2) sg2 = segs[blkmap[blk_off + b2]];
-        if (b + G >= n_blk) break;
-        b += G;
-        cur = nxt;
-#pragma unroll
-        for (int a = 0; a < 8; ++a) id[a] = idn[a];
-        if (has2) nxt = describe(b2, sg2); else nxt.cls = -1;
-    }
-}
-
 // natural [nf][NL] <-> block-shell [nf][GFS]; one thread per natural node, so the natural side
 // is coalesced and the shell side is a gather / scatter inside the block's record (run once
 // per numa_step_rk3 call, not per stage)
@@ -716,11 +621,7 @@ cudaError_t launch_dss_classes(numa_ctx *c, const DssLists &L, double *r, int64_
     if (nblk <= 0) return cudaSuccess;
     LaunchScope ls(c, kernel_id, s);
     const bool hi = c->par.N >= 6;   // measured: N=5 0.52 (10) vs 0.56 (16); N=6 0.45 vs 0.44; N=7 0.39 vs 0.36; N=8 0.37 vs 0.34 ms
-#ifndef NUMA_DSS_PIPE   /* measured slower than the one-shot kernel */
 #define DSS_LAUNCH(F, MB) k_stage_dss<F, MB><<<(unsigned)nblk, NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start, L.copies, stride, (int)blk0)
-#else
-#define DSS_LAUNCH(F, MB) k_stage_dss_pipe<F, (MB == NUMA_DSS_MINB_HI ? NUMA_DSS_PIPE_MINB_HI : NUMA_DSS_PIPE_MINB)><<<(unsigned)(nblk < (int64_t)c->n_sm * NUMA_DSS_PIPE_GRID ? nblk : (int64_t)c->n_sm * NUMA_DSS_PIPE_GRID), NUMA_DSS_THREADS, 0, s>>>(r, L.idx, L.seg, L.blkmap, L.sh_nodes, L.start, L.copies, stride, (int)blk0, (int)nblk)
-#endif
     if (nf == 5) { if (hi) DSS_LAUNCH(5, NUMA_DSS_MINB_HI); else DSS_LAUNCH(5, NUMA_DSS_MINB); }
     else if (nf == 4) { if (hi) DSS_LAUNCH(4, NUMA_DSS_MINB_HI); else DSS_LAUNCH(4, NUMA_DSS_MINB); }
     else return cudaErrorInvalidValue;
